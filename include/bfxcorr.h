@@ -1,0 +1,124 @@
+/* bfxcorr.h -- C ABI of the B200-native X-engine (cross-multiply-accumulate correlator stage).
+ *
+ * What the library computes (BASELINE.json `north_star`; the paper itself prints no formula for
+ * correlation: PAPER.md:141 lists a "Linear algebra -- matrix multiplication and related routines"
+ * back-end module and PAPER.md:579 lists "comprehensive support for correlation" as near-term work):
+ *
+ *   for every channel c and every input pair i >= j (autocorrelations i == j included)
+ *       V[c][i][j]  =  sum over the span's ntime samples t of   x[t][c][i] * conj( x[t][c][j] )
+ *         .re = sum_t ( re_i*re_j + im_i*im_j )
+ *         .im = sum_t ( im_i*re_j - re_i*im_j )
+ *       out[c][ i*(i+1)/2 + j ]  =  (accumulate ? out[...] : 0) + V[c][i][j]
+ *
+ * i.e. the lower triangle of the Hermitian visibility matrix V[c] += sum_t x_t x_t^H, kept in int32
+ * complex accumulators that persist across successive ring-buffer spans (PAPER.md:165 spans,
+ * PAPER.md:345 "every span is contiguous", "Accumulate frames one at a time").
+ *
+ * Data formats (DESIGN.md section 3 lists every reading the paper leaves open):
+ *   input  `in`  : DEVICE pointer, one dense span [ntime][nchan][ninputs], input index fastest.
+ *       BF_XCORR_CI8 ("8+8 bit complex"): 2 bytes per sample, byte 0 = re, byte 1 = im,
+ *                    both two's-complement int8; the code -128 is legal.
+ *       BF_XCORR_CI4 ("4+4 complex signed integers"): 1 byte per sample,
+ *                    re = high nibble (bits 7..4), im = low nibble (bits 3..0), each two's
+ *                    complement in [-8, 7]; the code -8 is legal.
+ *   output `out` : DEVICE pointer, [nchan][B][2] int32 with B = ninputs*(ninputs+1)/2; element
+ *                  k = i*(i+1)/2 + j (row-major packed lower triangle, i >= j) holds (re, im).
+ *   Arithmetic   : exact integer; int32 accumulators wrap modulo 2^32 (no saturation).  With
+ *                  |re|,|im| <= 128 (ci8) a visibility cannot wrap before 65 535 accumulated samples
+ *                  (bfXcorrGetMaxSafeNtime); ci4: 16 777 215.
+ *
+ * Ownership and ordering: the caller owns `in`, `out` and the stream.  bfXcorrExecute only enqueues
+ * work on `stream` and returns without synchronising; `in` and `out` must stay valid until the stream
+ * reaches that point.  The plan owns its private device scratch (descriptors, work tables), allocated
+ * by bfXcorrCreate on the CUDA device that is current at that call and released by bfXcorrDestroy.
+ * A plan may be used by one host thread at a time.  Results are deterministic (integer sums).
+ *
+ * Errors: every entry point returns a bfXcorrStatus (0 = OK); nothing aborts or throws across the ABI.
+ * There is NO CPU fallback: without a compute-capability-10.x device bfXcorrCreate returns
+ * BF_XCORR_UNSUPPORTED_DEVICE.
+ */
+#ifndef BFXCORR_H_
+#define BFXCORR_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct bfXcorr_impl* bfXcorr; /* opaque plan handle */
+
+typedef enum bfXcorrDtype_ {
+    BF_XCORR_CI4 = 4, /* 4+4-bit complex */
+    BF_XCORR_CI8 = 8  /* 8+8-bit complex */
+} bfXcorrDtype;
+
+typedef enum bfXcorrStatus_ {
+    BF_XCORR_OK = 0,
+    BF_XCORR_INVALID_POINTER = 1,    /* NULL plan/in/out/result pointer, or misaligned in/out */
+    BF_XCORR_INVALID_HANDLE = 2,     /* NULL or already destroyed plan */
+    BF_XCORR_INVALID_ARGUMENT = 3,   /* non-positive dimension, unknown algorithm, ...         */
+    BF_XCORR_INVALID_DTYPE = 4,      /* dtype not BF_XCORR_CI4 / BF_XCORR_CI8                   */
+    BF_XCORR_UNSUPPORTED_SHAPE = 5,  /* see bfXcorrCreate                                       */
+    BF_XCORR_UNSUPPORTED_DEVICE = 6, /* no CUDA device of compute capability 10.x               */
+    BF_XCORR_MEM_ALLOC_FAILED = 7,
+    BF_XCORR_DEVICE_ERROR = 8        /* a CUDA call failed; see bfXcorrGetLastCudaError         */
+} bfXcorrStatus;
+
+/* Which kernel bfXcorrExecute launches.  TCGEN05 is the product path and the default: TMA-staged
+ * int8 operands, tcgen05.mma kind::i8 with int32 accumulators held in TMEM over the whole span,
+ * lower-triangle tile scheduler, span-accumulate epilogue.  SIMT is a plain CUDA-core kernel kept as
+ * an on-device cross-check of the tensor path at sizes the CPU oracle cannot reach; it is never
+ * selected implicitly. */
+typedef enum bfXcorrAlgo_ {
+    BF_XCORR_ALGO_TCGEN05 = 0,
+    BF_XCORR_ALGO_SIMT = 1
+} bfXcorrAlgo;
+
+/* Create a plan for spans of exactly `ntime` samples x `nchan` channels x `ninputs` inputs of `dtype`
+ * (BASELINE.json north_star: bfXcorrCreate(ninputs, nchan, ntime, dtype)).
+ *   *plan  : receives the handle (host pointer, must not be NULL).
+ *   errors : INVALID_POINTER (plan NULL); INVALID_ARGUMENT (a dimension <= 0, or ntime > 65535);
+ *            INVALID_DTYPE; UNSUPPORTED_SHAPE (ninputs * bytes_per_sample not a multiple of 16: the
+ *            16-byte vector / TMA row granularity -- every BASELINE.json config satisfies it);
+ *            UNSUPPORTED_DEVICE; MEM_ALLOC_FAILED; DEVICE_ERROR. */
+int bfXcorrCreate(bfXcorr* plan, int ninputs, int nchan, int ntime, int dtype);
+
+/* Correlate one span (BASELINE.json north_star: bfXcorrExecute(in, out, accumulate, stream)).
+ *   in         : device pointer to the span, 16-byte aligned, bfXcorrGetInputBytes bytes, read only.
+ *   out        : device pointer to the visibilities, 16-byte aligned, bfXcorrGetOutputBytes bytes.
+ *   accumulate : 0 = overwrite `out` (it need not be initialised); non-zero = out += this span.
+ *   stream     : a cudaStream_t passed as void* (NULL = the legacy default stream).
+ *   errors     : INVALID_HANDLE; INVALID_POINTER (NULL or misaligned); DEVICE_ERROR (launch failed). */
+int bfXcorrExecute(bfXcorr plan, const void* in, void* out, int accumulate, void* stream);
+
+/* Release the plan and its device scratch.  errors: INVALID_HANDLE (NULL). */
+int bfXcorrDestroy(bfXcorr plan);
+
+/* Pure queries; `nbytes` / `nt` are host pointers.  errors: INVALID_HANDLE, INVALID_POINTER. */
+int bfXcorrGetInputBytes(bfXcorr plan, unsigned long long* nbytes);  /* ntime*nchan*ninputs*(1|2)   */
+int bfXcorrGetOutputBytes(bfXcorr plan, unsigned long long* nbytes); /* nchan*ninputs*(ninputs+1)/2*8 */
+int bfXcorrGetMaxSafeNtime(bfXcorr plan, unsigned long long* nt);    /* samples before int32 may wrap */
+
+/* Select the kernel (see bfXcorrAlgo).  errors: INVALID_HANDLE, INVALID_ARGUMENT. */
+int bfXcorrSetAlgo(bfXcorr plan, int algo);
+
+/* Number of kernels the last bfXcorrExecute on this plan launched (for launch accounting). */
+int bfXcorrGetLaunchCount(bfXcorr plan, int* nlaunch);
+
+/* cudaError_t of the last failing CUDA call made on behalf of this plan (0 if none). */
+int bfXcorrGetLastCudaError(bfXcorr plan, int* cuda_error);
+
+/* Convenience for callers whose buffers live in HOST memory (bench.py's end-to-end leg): copies the
+ * span host->device into plan-owned staging, executes, and -- if `out_host` is not NULL -- copies the
+ * visibility buffer device->host, all on `stream`; `out_dev` is the persistent device accumulator.
+ *   in_host, out_host : HOST pointers (pinned memory makes the copies asynchronous).
+ *   errors            : as bfXcorrExecute, plus MEM_ALLOC_FAILED for the staging buffer. */
+int bfXcorrExecuteHost(bfXcorr plan, const void* in_host, void* out_dev, void* out_host, int accumulate,
+                       void* stream);
+
+/* Static string for a status code (never NULL). */
+const char* bfXcorrGetStatusString(int status);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BFXCORR_H_ */

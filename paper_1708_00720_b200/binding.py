@@ -1,0 +1,125 @@
+"""ctypes binding of include/bfxcorr.h -- argument marshalling only.
+
+Same names as the C ABI.  Every step of the hot path (unpack, tile scheduling, tensor-core
+contraction, span-accumulate epilogue) runs inside libbfxcorr.so's CUDA kernels; this module never
+computes anything and never falls back to a CPU implementation: if the library cannot be built or
+loaded, importing callers get an exception.  torch is used by callers for device memory and streams.
+"""
+from __future__ import annotations
+
+import ctypes
+from typing import Optional
+
+from . import _build
+
+BF_XCORR_CI4 = 4
+BF_XCORR_CI8 = 8
+BF_XCORR_OK = 0
+BF_XCORR_ALGO_TCGEN05 = 0
+BF_XCORR_ALGO_SIMT = 1
+
+_vp = ctypes.c_void_p
+_i = ctypes.c_int
+_ullp = ctypes.POINTER(ctypes.c_ulonglong)
+_ip = ctypes.POINTER(ctypes.c_int)
+
+# name -> (restype, argtypes); mirrors include/bfxcorr.h one to one
+SIGNATURES = {
+    "bfXcorrCreate": (_i, [ctypes.POINTER(_vp), _i, _i, _i, _i]),
+    "bfXcorrExecute": (_i, [_vp, _vp, _vp, _i, _vp]),
+    "bfXcorrDestroy": (_i, [_vp]),
+    "bfXcorrGetInputBytes": (_i, [_vp, _ullp]),
+    "bfXcorrGetOutputBytes": (_i, [_vp, _ullp]),
+    "bfXcorrGetMaxSafeNtime": (_i, [_vp, _ullp]),
+    "bfXcorrSetAlgo": (_i, [_vp, _i]),
+    "bfXcorrGetLaunchCount": (_i, [_vp, _ip]),
+    "bfXcorrGetLastCudaError": (_i, [_vp, _ip]),
+    "bfXcorrExecuteHost": (_i, [_vp, _vp, _vp, _vp, _i, _vp]),
+    "bfXcorrGetStatusString": (ctypes.c_char_p, [_i]),
+}
+
+_LIB: Optional[ctypes.CDLL] = None
+
+
+def lib() -> ctypes.CDLL:
+    """Load (building if needed) libbfxcorr.so and declare every prototype."""
+    global _LIB
+    if _LIB is None:
+        handle = ctypes.CDLL(_build.build())
+        for name, (res, args) in SIGNATURES.items():
+            fn = getattr(handle, name)
+            fn.restype = res
+            fn.argtypes = args
+        _LIB = handle
+    return _LIB
+
+
+class BfXcorrError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        super().__init__("%s failed: %s (%d)" % (where, bfXcorrGetStatusString(status), status))
+
+
+def _check(status: int, where: str) -> None:
+    if status != BF_XCORR_OK:
+        raise BfXcorrError(status, where)
+
+
+def bfXcorrGetStatusString(status: int) -> str:
+    return lib().bfXcorrGetStatusString(int(status)).decode()
+
+
+def bfXcorrCreate(ninputs: int, nchan: int, ntime: int, dtype: int) -> _vp:
+    plan = _vp()
+    _check(lib().bfXcorrCreate(ctypes.byref(plan), ninputs, nchan, ntime, dtype), "bfXcorrCreate")
+    return plan
+
+
+def bfXcorrExecute(plan: _vp, in_ptr: int, out_ptr: int, accumulate: bool, stream: int = 0) -> None:
+    """in_ptr / out_ptr: device addresses (tensor.data_ptr()); stream: cudaStream_t as int."""
+    _check(lib().bfXcorrExecute(plan, _vp(in_ptr), _vp(out_ptr), 1 if accumulate else 0, _vp(stream)),
+           "bfXcorrExecute")
+
+
+def bfXcorrExecuteHost(plan: _vp, in_host_ptr: int, out_dev_ptr: int, out_host_ptr: int, accumulate: bool,
+                       stream: int = 0) -> None:
+    _check(lib().bfXcorrExecuteHost(plan, _vp(in_host_ptr), _vp(out_dev_ptr), _vp(out_host_ptr or None),
+                                    1 if accumulate else 0, _vp(stream)), "bfXcorrExecuteHost")
+
+
+def bfXcorrDestroy(plan: _vp) -> None:
+    _check(lib().bfXcorrDestroy(plan), "bfXcorrDestroy")
+
+
+def _get_ull(fn_name: str, plan: _vp) -> int:
+    v = ctypes.c_ulonglong(0)
+    _check(getattr(lib(), fn_name)(plan, ctypes.byref(v)), fn_name)
+    return int(v.value)
+
+
+def bfXcorrGetInputBytes(plan: _vp) -> int:
+    return _get_ull("bfXcorrGetInputBytes", plan)
+
+
+def bfXcorrGetOutputBytes(plan: _vp) -> int:
+    return _get_ull("bfXcorrGetOutputBytes", plan)
+
+
+def bfXcorrGetMaxSafeNtime(plan: _vp) -> int:
+    return _get_ull("bfXcorrGetMaxSafeNtime", plan)
+
+
+def bfXcorrSetAlgo(plan: _vp, algo: int) -> None:
+    _check(lib().bfXcorrSetAlgo(plan, algo), "bfXcorrSetAlgo")
+
+
+def bfXcorrGetLaunchCount(plan: _vp) -> int:
+    v = ctypes.c_int(0)
+    _check(lib().bfXcorrGetLaunchCount(plan, ctypes.byref(v)), "bfXcorrGetLaunchCount")
+    return int(v.value)
+
+
+def bfXcorrGetLastCudaError(plan: _vp) -> int:
+    v = ctypes.c_int(0)
+    _check(lib().bfXcorrGetLastCudaError(plan, ctypes.byref(v)), "bfXcorrGetLastCudaError")
+    return int(v.value)

@@ -1,0 +1,324 @@
+// bfxcorr.cu -- host side of the C ABI declared in include/bfxcorr.h: plan construction (tile table,
+// TMA tensor map), launch of the sm_100a kernels, status codes.  No CPU compute path exists here.
+#include <cstdint>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include "../../include/bfxcorr.h"
+#include "xcorr_simt.cuh"
+#include "xcorr_tcgen05.cuh"
+
+namespace {
+
+using bfx::TcCfg;
+using bfx::TcParams;
+using bfx::TcTile;
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+constexpr uint32_t kMagic = 0xBFC0DE01u;
+
+}  // namespace
+
+struct bfXcorr_impl {
+    uint32_t magic;
+    int ninputs, nchan, ntime, dtype;
+    int algo;
+    int device;
+    int num_sms;
+    int last_cuda_error;
+    int last_launch_count;
+    // S2: lower-triangle tile table (device copy) for the tcgen05 kernel
+    TcTile* d_tiles;
+    int tiles_per_chan;
+    EncodeTiledFn encode;
+    // staging for bfXcorrExecuteHost
+    void* d_stage_in;
+};
+
+namespace {
+
+bool valid(bfXcorr p) { return p != nullptr && p->magic == kMagic; }
+
+int cuda_fail(bfXcorr p, cudaError_t e)
+{
+    if (p) p->last_cuda_error = static_cast<int>(e);
+    return e == cudaErrorMemoryAllocation ? BF_XCORR_MEM_ALLOC_FAILED : BF_XCORR_DEVICE_ERROR;
+}
+
+unsigned long long bytes_per_sample(int dtype) { return dtype == BF_XCORR_CI4 ? 1ull : 2ull; }
+
+unsigned long long input_bytes(bfXcorr p)
+{
+    return static_cast<unsigned long long>(p->ntime) * p->nchan * p->ninputs * bytes_per_sample(p->dtype);
+}
+
+unsigned long long output_bytes(bfXcorr p)
+{
+    const unsigned long long n = p->ninputs;
+    return static_cast<unsigned long long>(p->nchan) * (n * (n + 1) / 2) * 8ull;
+}
+
+// S2: enumerate only the tiles that touch the lower triangle.  Row blocks are 64
+// inputs (UMMA M = 128 real rows), column blocks 128 inputs (UMMA N = 256); a tile whose second 64-input
+// column half lies wholly above the diagonal (or beyond N) is issued with N = 128.
+std::vector<TcTile> build_tiles(int ninputs)
+{
+    std::vector<TcTile> tiles;
+    const int nrb = (ninputs + bfx::TC_BM_IN - 1) / bfx::TC_BM_IN;
+    for (int r = 0; r < nrb; ++r) {
+        const int i0 = r * bfx::TC_BM_IN;
+        const int i_last = (i0 + bfx::TC_BM_IN < ninputs ? i0 + bfx::TC_BM_IN : ninputs) - 1;
+        for (int cb = 0; cb * bfx::TC_BN_IN <= i_last; ++cb) {
+            const int j0 = cb * bfx::TC_BN_IN;
+            TcTile t;
+            t.row_blk = static_cast<int16_t>(r);
+            t.col_blk = static_cast<int16_t>(cb);
+            t.nbox = static_cast<int8_t>((j0 + 64 <= i_last) ? 2 : 1);
+            const int d = (i0 - j0) / 64;
+            t.a_alias = static_cast<int8_t>((i0 >= j0 && d < t.nbox) ? d : -1);
+            t.pad = 0;
+            tiles.push_back(t);
+        }
+    }
+    return tiles;
+}
+
+int make_tensor_map(bfXcorr p, const void* in, CUtensorMap* tmap)
+{
+    // span as a 3-D byte tensor, innermost first: (row bytes, nchan, ntime)
+    const unsigned long long row = static_cast<unsigned long long>(p->ninputs) * bytes_per_sample(p->dtype);
+    const cuuint64_t dims[3] = {row, static_cast<cuuint64_t>(p->nchan), static_cast<cuuint64_t>(p->ntime)};
+    const cuuint64_t strides[2] = {row, row * static_cast<cuuint64_t>(p->nchan)};
+    const cuuint32_t box[3] = {p->dtype == BF_XCORR_CI4 ? 64u : 128u, 1u, static_cast<cuuint32_t>(bfx::TC_KT)};
+    const cuuint32_t estr[3] = {1u, 1u, 1u};
+    const CUresult r = p->encode(tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<void*>(in), dims, strides, box, estr,
+                                 CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                 p->dtype == BF_XCORR_CI4 ? CU_TENSOR_MAP_SWIZZLE_NONE : CU_TENSOR_MAP_SWIZZLE_128B,
+                                 CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        p->last_cuda_error = static_cast<int>(cudaErrorInvalidValue);
+        return BF_XCORR_DEVICE_ERROR;
+    }
+    return BF_XCORR_OK;
+}
+
+template <bool CI4>
+int launch_tcgen05(bfXcorr p, const void* in, void* out, int accumulate, cudaStream_t stream)
+{
+    CUtensorMap tmap;
+    const int st = make_tensor_map(p, in, &tmap);
+    if (st != BF_XCORR_OK) return st;
+    TcParams prm;
+    prm.out = static_cast<int32_t*>(out);
+    prm.tiles = p->d_tiles;
+    prm.ninputs = p->ninputs;
+    prm.nchan = p->nchan;
+    prm.ntime = p->ntime;
+    prm.tiles_per_chan = p->tiles_per_chan;
+    prm.ntiles = static_cast<long long>(p->tiles_per_chan) * p->nchan;
+    prm.accumulate = accumulate ? 1 : 0;
+    const long long want = prm.ntiles < p->num_sms ? prm.ntiles : p->num_sms;
+    const dim3 grid(static_cast<unsigned>(want));
+    bfx::xcorr_tcgen05_kernel<CI4><<<grid, TcCfg<CI4>::kThreads, TcCfg<CI4>::kSmemBytes, stream>>>(tmap, prm);
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(p, e);
+    p->last_launch_count = 1;
+    return BF_XCORR_OK;
+}
+
+int launch_simt(bfXcorr p, const void* in, void* out, int accumulate, cudaStream_t stream)
+{
+    const int nb = (p->ninputs + bfx::SIMT_TILE - 1) / bfx::SIMT_TILE;
+    const dim3 grid(static_cast<unsigned>(nb * (nb + 1) / 2), static_cast<unsigned>(p->nchan < 65535 ? p->nchan : 65535));
+    bfx::xcorr_simt_kernel<<<grid, 256, 0, stream>>>(static_cast<const uint8_t*>(in), static_cast<int32_t*>(out),
+                                                     p->ninputs, p->nchan, p->ntime, p->dtype, accumulate ? 1 : 0);
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(p, e);
+    p->last_launch_count = 1;
+    return BF_XCORR_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int bfXcorrCreate(bfXcorr* plan, int ninputs, int nchan, int ntime, int dtype)
+{
+    if (!plan) return BF_XCORR_INVALID_POINTER;
+    *plan = nullptr;
+    if (ninputs <= 0 || nchan <= 0 || ntime <= 0 || ntime > 65535) return BF_XCORR_INVALID_ARGUMENT;
+    if (dtype != BF_XCORR_CI4 && dtype != BF_XCORR_CI8) return BF_XCORR_INVALID_DTYPE;
+    if ((static_cast<unsigned long long>(ninputs) * bytes_per_sample(dtype)) % 16ull != 0) return BF_XCORR_UNSUPPORTED_SHAPE;
+    if (ninputs > 32768) return BF_XCORR_UNSUPPORTED_SHAPE;
+
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev <= 0) {
+        cudaGetLastError();
+        return BF_XCORR_UNSUPPORTED_DEVICE;
+    }
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return BF_XCORR_UNSUPPORTED_DEVICE;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return BF_XCORR_UNSUPPORTED_DEVICE;
+    if (prop.major != 10) return BF_XCORR_UNSUPPORTED_DEVICE;
+
+    bfXcorr p = new (std::nothrow) bfXcorr_impl;
+    if (!p) return BF_XCORR_MEM_ALLOC_FAILED;
+    std::memset(p, 0, sizeof(*p));
+    p->magic = kMagic;
+    p->ninputs = ninputs;
+    p->nchan = nchan;
+    p->ntime = ntime;
+    p->dtype = dtype;
+    p->algo = BF_XCORR_ALGO_TCGEN05;
+    p->device = dev;
+    p->num_sms = prop.multiProcessorCount;
+
+    // cuTensorMapEncodeTiled through the runtime's driver entry point (no link-time libcuda dependency)
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+    if (e != cudaSuccess || qres != cudaDriverEntryPointSuccess || !fn) {
+        delete p;
+        return BF_XCORR_UNSUPPORTED_DEVICE;
+    }
+    p->encode = reinterpret_cast<EncodeTiledFn>(fn);
+
+    const std::vector<TcTile> tiles = build_tiles(ninputs);
+    p->tiles_per_chan = static_cast<int>(tiles.size());
+    e = cudaMalloc(reinterpret_cast<void**>(&p->d_tiles), tiles.size() * sizeof(TcTile));
+    if (e == cudaSuccess) e = cudaMemcpy(p->d_tiles, tiles.data(), tiles.size() * sizeof(TcTile), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(bfx::xcorr_tcgen05_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 TcCfg<false>::kSmemBytes);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(bfx::xcorr_tcgen05_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 TcCfg<true>::kSmemBytes);
+    if (e != cudaSuccess) {
+        const int st = cuda_fail(nullptr, e);
+        if (p->d_tiles) cudaFree(p->d_tiles);
+        delete p;
+        return st;
+    }
+    *plan = p;
+    return BF_XCORR_OK;
+}
+
+int bfXcorrExecute(bfXcorr plan, const void* in, void* out, int accumulate, void* stream)
+{
+    if (!valid(plan)) return BF_XCORR_INVALID_HANDLE;
+    if (!in || !out) return BF_XCORR_INVALID_POINTER;
+    if ((reinterpret_cast<uintptr_t>(in) & 15u) || (reinterpret_cast<uintptr_t>(out) & 15u)) return BF_XCORR_INVALID_POINTER;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    plan->last_launch_count = 0;
+    if (plan->algo == BF_XCORR_ALGO_SIMT) return launch_simt(plan, in, out, accumulate, s);
+    return plan->dtype == BF_XCORR_CI4 ? launch_tcgen05<true>(plan, in, out, accumulate, s)
+                                       : launch_tcgen05<false>(plan, in, out, accumulate, s);
+}
+
+int bfXcorrExecuteHost(bfXcorr plan, const void* in_host, void* out_dev, void* out_host, int accumulate, void* stream)
+{
+    if (!valid(plan)) return BF_XCORR_INVALID_HANDLE;
+    if (!in_host || !out_dev) return BF_XCORR_INVALID_POINTER;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    cudaError_t e;
+    if (!plan->d_stage_in) {
+        e = cudaMalloc(&plan->d_stage_in, input_bytes(plan));
+        if (e != cudaSuccess) return cuda_fail(plan, e);
+    }
+    e = cudaMemcpyAsync(plan->d_stage_in, in_host, input_bytes(plan), cudaMemcpyHostToDevice, s);
+    if (e != cudaSuccess) return cuda_fail(plan, e);
+    const int st = bfXcorrExecute(plan, plan->d_stage_in, out_dev, accumulate, stream);
+    if (st != BF_XCORR_OK) return st;
+    if (out_host) {
+        e = cudaMemcpyAsync(out_host, out_dev, output_bytes(plan), cudaMemcpyDeviceToHost, s);
+        if (e != cudaSuccess) return cuda_fail(plan, e);
+    }
+    return BF_XCORR_OK;
+}
+
+int bfXcorrDestroy(bfXcorr plan)
+{
+    if (!valid(plan)) return BF_XCORR_INVALID_HANDLE;
+    if (plan->d_tiles) cudaFree(plan->d_tiles);
+    if (plan->d_stage_in) cudaFree(plan->d_stage_in);
+    plan->magic = 0;
+    delete plan;
+    return BF_XCORR_OK;
+}
+
+int bfXcorrGetInputBytes(bfXcorr plan, unsigned long long* nbytes)
+{
+    if (!valid(plan)) return BF_XCORR_INVALID_HANDLE;
+    if (!nbytes) return BF_XCORR_INVALID_POINTER;
+    *nbytes = input_bytes(plan);
+    return BF_XCORR_OK;
+}
+
+int bfXcorrGetOutputBytes(bfXcorr plan, unsigned long long* nbytes)
+{
+    if (!valid(plan)) return BF_XCORR_INVALID_HANDLE;
+    if (!nbytes) return BF_XCORR_INVALID_POINTER;
+    *nbytes = output_bytes(plan);
+    return BF_XCORR_OK;
+}
+
+int bfXcorrGetMaxSafeNtime(bfXcorr plan, unsigned long long* nt)
+{
+    if (!valid(plan)) return BF_XCORR_INVALID_HANDLE;
+    if (!nt) return BF_XCORR_INVALID_POINTER;
+    // |Re V| <= samples * 2 m^2 with m = 128 (ci8) or 8 (ci4); must stay <= 2^31 - 1
+    const unsigned long long m = plan->dtype == BF_XCORR_CI4 ? 8ull : 128ull;
+    *nt = 2147483647ull / (2ull * m * m);
+    return BF_XCORR_OK;
+}
+
+int bfXcorrSetAlgo(bfXcorr plan, int algo)
+{
+    if (!valid(plan)) return BF_XCORR_INVALID_HANDLE;
+    if (algo != BF_XCORR_ALGO_TCGEN05 && algo != BF_XCORR_ALGO_SIMT) return BF_XCORR_INVALID_ARGUMENT;
+    plan->algo = algo;
+    return BF_XCORR_OK;
+}
+
+int bfXcorrGetLaunchCount(bfXcorr plan, int* nlaunch)
+{
+    if (!valid(plan)) return BF_XCORR_INVALID_HANDLE;
+    if (!nlaunch) return BF_XCORR_INVALID_POINTER;
+    *nlaunch = plan->last_launch_count;
+    return BF_XCORR_OK;
+}
+
+int bfXcorrGetLastCudaError(bfXcorr plan, int* cuda_error)
+{
+    if (!valid(plan)) return BF_XCORR_INVALID_HANDLE;
+    if (!cuda_error) return BF_XCORR_INVALID_POINTER;
+    *cuda_error = plan->last_cuda_error;
+    return BF_XCORR_OK;
+}
+
+const char* bfXcorrGetStatusString(int status)
+{
+    switch (status) {
+        case BF_XCORR_OK: return "BF_XCORR_OK";
+        case BF_XCORR_INVALID_POINTER: return "BF_XCORR_INVALID_POINTER";
+        case BF_XCORR_INVALID_HANDLE: return "BF_XCORR_INVALID_HANDLE";
+        case BF_XCORR_INVALID_ARGUMENT: return "BF_XCORR_INVALID_ARGUMENT";
+        case BF_XCORR_INVALID_DTYPE: return "BF_XCORR_INVALID_DTYPE";
+        case BF_XCORR_UNSUPPORTED_SHAPE: return "BF_XCORR_UNSUPPORTED_SHAPE";
+        case BF_XCORR_UNSUPPORTED_DEVICE: return "BF_XCORR_UNSUPPORTED_DEVICE";
+        case BF_XCORR_MEM_ALLOC_FAILED: return "BF_XCORR_MEM_ALLOC_FAILED";
+        case BF_XCORR_DEVICE_ERROR: return "BF_XCORR_DEVICE_ERROR";
+        default: return "BF_XCORR_UNKNOWN_STATUS";
+    }
+}
+
+}  // extern "C"

@@ -1,0 +1,141 @@
+"""`-m gpu` parity tests: the CUDA path (through the C ABI of include/bfxcorr.h) against the CPU
+oracle, element by element, BIT-EXACT (the path is integer-only with int32 accumulation:
+BASELINE.json north_star).  Sizes here are ones the oracle finishes in seconds and that span several
+tiles (64-input row blocks, 128-input column blocks, 64-sample pipeline stages) plus ragged tails."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import paper_1708_00720_b200 as bfx
+from gpu_harness import run_spans
+from helpers import pack, read_golden, tri_index
+from xcorr_inputs import CONFIGS, generate_span
+
+pytestmark = pytest.mark.gpu
+
+ALGOS = [bfx.BF_XCORR_ALGO_TCGEN05, bfx.BF_XCORR_ALGO_SIMT]
+ALGO_IDS = ["tcgen05", "simt"]
+
+
+def rand_span(rng, T, C, N, dtype):
+    lo, hi = (-8, 7) if dtype == 4 else (-128, 127)
+    re = rng.integers(lo, hi + 1, size=(T, C, N))
+    im = rng.integers(lo, hi + 1, size=(T, C, N))
+    return pack(dtype, re, im)
+
+
+# shapes: (ninputs, nchan, ntime); every ninputs*bytes_per_sample is a multiple of 16
+SHAPES_CI8 = [(16, 4, 256), (8, 3, 7), (64, 5, 100), (80, 2, 64), (128, 3, 96), (136, 2, 65), (192, 2, 130),
+              (256, 2, 33), (320, 1, 200), (512, 2, 64), (520, 1, 40)]
+SHAPES_CI4 = [(16, 3, 40), (64, 4, 129), (96, 2, 64), (128, 3, 31), (208, 2, 70), (256, 1, 128), (512, 1, 96)]
+
+
+@pytest.mark.parametrize("algo", ALGOS, ids=ALGO_IDS)
+@pytest.mark.parametrize("shape", SHAPES_CI8, ids=lambda s: "n%dc%dt%d" % s)
+def test_random_ci8_bit_exact(shape, algo):
+    N, C, T = shape
+    x = rand_span(np.random.default_rng(1000 + N + T), T, C, N, 8)
+    got = run_spans([x], N, C, T, 8, algo)
+    np.testing.assert_array_equal(got, oracle.xcorr(x, N, C, T, 8))
+
+
+@pytest.mark.parametrize("algo", ALGOS, ids=ALGO_IDS)
+@pytest.mark.parametrize("shape", SHAPES_CI4, ids=lambda s: "n%dc%dt%d" % s)
+def test_random_ci4_bit_exact(shape, algo):
+    N, C, T = shape
+    x = rand_span(np.random.default_rng(2000 + N + T), T, C, N, 4)
+    got = run_spans([x], N, C, T, 4, algo)
+    np.testing.assert_array_equal(got, oracle.xcorr(x, N, C, T, 4))
+
+
+@pytest.mark.parametrize("algo", ALGOS, ids=ALGO_IDS)
+@pytest.mark.parametrize("name", ["worked_example_n3.txt", "worked_example_n2.txt"])
+@pytest.mark.parametrize("dtype", [4, 8])
+def test_worked_examples_embedded(name, dtype, algo):
+    """tests/golden hand-worked values, zero-padded to the 16-byte row granularity."""
+    g = read_golden(name)
+    T = 1 + max(t for t, _, _, _ in g["x"])
+    N = 16
+    re = np.zeros((T, 1, N), dtype=np.int64)
+    im = np.zeros((T, 1, N), dtype=np.int64)
+    for t, i, r, m in g["x"]:
+        re[t, 0, i], im[t, 0, i] = r, m
+    got = run_spans([pack(dtype, re, im)], N, 1, T, dtype, algo)
+    exp = np.zeros_like(got)
+    n_small = 1 + max(i for _, i, _, _ in g["x"])
+    k = 0
+    for i in range(n_small):
+        for j in range(i + 1):
+            _, vr, vi = g["v"][k]
+            exp[0, tri_index(i, j)] = (vr, vi)
+            k += 1
+    np.testing.assert_array_equal(got, exp)
+
+
+@pytest.mark.parametrize("algo", ALGOS, ids=ALGO_IDS)
+@pytest.mark.parametrize("dtype", [4, 8])
+def test_extreme_codes(dtype, algo):
+    """All samples at the most negative code (-128-128j / -8-8j): reading A6, must stay exact."""
+    N, C, T = 144, 2, 100
+    m = -8 if dtype == 4 else -128
+    re = np.full((T, C, N), m, dtype=np.int64)
+    x = pack(dtype, re, re)
+    got = run_spans([x], N, C, T, dtype, algo)
+    assert (got[..., 0] == 2 * m * m * T).all() and (got[..., 1] == 0).all()
+
+
+@pytest.mark.parametrize("algo", ALGOS, ids=ALGO_IDS)
+@pytest.mark.parametrize("dtype", [4, 8])
+def test_accumulation_laws(dtype, algo):
+    """Spans accumulate: three spans == oracle of three spans; accumulate=0 ignores
+    what is in `out`; one span of 2T == two spans of T."""
+    N, C, T = 192, 3, 70
+    rng = np.random.default_rng(77 + dtype)
+    xs = [rand_span(rng, T, C, N, dtype) for _ in range(3)]
+    exp = oracle.xcorr(xs[0], N, C, T, dtype)
+    for x in xs[1:]:
+        oracle.xcorr(x, N, C, T, dtype, out=exp, accumulate=True)
+    got = run_spans(xs, N, C, T, dtype, algo)
+    np.testing.assert_array_equal(got, exp)
+    both = np.concatenate(xs[:2], axis=0)
+    one = run_spans([both], N, C, 2 * T, dtype, algo)
+    two = run_spans(xs[:2], N, C, T, dtype, algo)
+    np.testing.assert_array_equal(one, two)
+
+
+@pytest.mark.parametrize("algo", ALGOS, ids=ALGO_IDS)
+def test_accumulate_into_existing_and_wraparound(algo):
+    """accumulate != 0 on the first call adds to the caller's buffer, wrapping mod 2^32 (reading A7)."""
+    N, C, T = 64, 2, 50
+    x = rand_span(np.random.default_rng(5), T, C, N, 8)
+    nb = N * (N + 1) // 2
+    init = torch.full((C, nb, 2), 2**31 - 5, dtype=torch.int32)
+    got = run_spans([x], N, C, T, 8, algo, first_accumulate=True, init=init)
+    exp = init.numpy().copy()
+    oracle.xcorr(x, N, C, T, 8, out=exp, accumulate=True)
+    np.testing.assert_array_equal(got, exp)
+
+
+def test_cfg1_tiny_config_bit_exact():
+    """BASELINE.json configs[0] exactly as generated for the bench."""
+    cfg = CONFIGS["cfg1"]
+    x = generate_span(cfg, 0).numpy()
+    for algo in ALGOS:
+        got = run_spans([x], cfg.ninputs, cfg.nchan, cfg.ntime, cfg.dtype, algo)
+        exp, nwrap = oracle.xcorr(x, cfg.ninputs, cfg.nchan, cfg.ntime, cfg.dtype, return_nwrap=True)
+        assert nwrap == 0
+        np.testing.assert_array_equal(got, exp)
+
+
+@pytest.mark.parametrize("dtype", [4, 8])
+def test_tcgen05_equals_simt_mid_size(dtype):
+    """Two independent device kernels agree bit for bit on a station-shaped (512-input) span."""
+    N, C, T = 512, 24, 256
+    x = rand_span(np.random.default_rng(9), T, C, N, dtype)
+    a = run_spans([x], N, C, T, dtype, bfx.BF_XCORR_ALGO_TCGEN05)
+    b = run_spans([x], N, C, T, dtype, bfx.BF_XCORR_ALGO_SIMT)
+    np.testing.assert_array_equal(a, b)
+    sub = [0, 11, 23]
+    exp = oracle.xcorr(np.ascontiguousarray(x[:, sub]), N, len(sub), T, dtype)
+    np.testing.assert_array_equal(a[sub], exp)
