@@ -1,0 +1,383 @@
+#!/usr/bin/env python
+"""bench.py -- X-engine throughput on B200 (BASELINE.json metric), one JSON line on stdout.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config cfg3] [--impl reference]
+
+A "step" is one pass of the whole hot path (S1 unpack/stage, S2 tile schedule, S3 tensor-core
+cross-multiply, S4 span-accumulate) over one batch of synthetic input: all spans of the config,
+the first with accumulate=0 and the rest accumulating into the persistent visibility buffer.
+Default workload: BASELINE.json configs[2] ("cfg3": 512 inputs, 3072 channels, 1024 samples, ci8,
+2 spans) -- the 512-input ci8 station config the north_star's target is quoted on.
+
+value       useful int8 TOPS = 8 * ntime * nchan * nbaselines * nspans / time, inputs resident in HBM
+e2e         same metric through bfXcorrExecuteHost: pinned HOST spans copied in and the visibility
+            buffer copied back inside the timed region
+roofline    dominant kernel (the only kernel): algorithmic ops (and bytes) per launch / mean launch
+            duration from CUDA events on the launching stream, against MEASURED_PEAKS.json
+cpu_baseline the CPU oracle (oracle/, as it stands) timed on this box's host cores on a bounded
+            sample of the same workload -- a baseline, not the target
+N > 1       channels are independent: every rank runs the same per-GPU workload on
+            its own GPU with no collective on the data path ("weak" scaling); time = max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "X-engine int8 TOPS (useful ops: 8 per complex MAC, lower triangle incl. autos)"
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            p = json.load(f)
+        return {"hbm_gbs": float(p["hbm_gbs"]), "bf16_burst": float(p["bf16_tflops"]),
+                "bf16_sustained": float(p.get("bf16_tflops_sustained", p["bf16_tflops"])), "source": "measured"}
+    # fallback stated in the B200 profiling recipe
+    return {"hbm_gbs": 6650.0, "bf16_burst": 1590.0, "bf16_sustained": 1400.0, "source": "fallback"}
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.rows = []
+        self.proc = None
+        self.gpu = gpu_index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.gpu), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits", "-lms", "50"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.06)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        sm_sorted = sorted(sm)
+        return {"sm_mhz": sm_sorted[len(sm_sorted) // 2], "sm_max_mhz": max(mx), "power_w_max": max(pw),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def workload_numbers(cfg):
+    nb = cfg.nbaselines
+    ops_span = 8.0 * cfg.ntime * cfg.nchan * nb
+    samples_span = float(cfg.ntime) * cfg.nchan * cfg.ninputs
+    in_bytes = float(cfg.span_bytes)
+    out_bytes = float(cfg.out_bytes)
+    # algorithmic bytes: span read once, visibilities written once (+ read once when accumulating)
+    bytes_all = cfg.nspans * in_bytes + out_bytes + (cfg.nspans - 1) * 2 * out_bytes
+    return dict(ops_span=ops_span, samples_span=samples_span, in_bytes=in_bytes, out_bytes=out_bytes,
+                ops_step=ops_span * cfg.nspans, samples_step=samples_span * cfg.nspans, bytes_step=bytes_all)
+
+
+def config_dict(cfg, extra=None):
+    d = {"workload": "%s: %d inputs x %d channels x %d samples, ci%d, %d span(s) per step (BASELINE.json configs[%d])" % (
+        cfg.name, cfg.ninputs, cfg.nchan, cfg.ntime, cfg.dtype, cfg.nspans, int(cfg.name[3:]) - 1),
+        "ninputs": cfg.ninputs, "nchan": cfg.nchan, "ntime": cfg.ntime, "dtype": "ci%d" % cfg.dtype,
+        "nspans": cfg.nspans, "seed": cfg.seed}
+    if extra:
+        d.update(extra)
+    return d
+
+
+def oracle_sample(cfg, target_s: float):
+    """Time the oracle (as it stands) on a bounded channel subset of the workload.
+    Returns (seconds, nchannels_used, threads)."""
+    import numpy as np
+    import oracle
+    from xcorr_inputs import generate_channel_slab
+    nthreads = oracle.threads()
+    # calibration: one channel per thread, one span
+    ncal = min(cfg.nchan, nthreads)
+    chans = [int(round(k * (cfg.nchan - 1) / max(1, ncal - 1))) for k in range(ncal)] if ncal > 1 else [0]
+    x = generate_channel_slab(cfg, 0, chans).numpy()
+    t0 = time.perf_counter()
+    oracle.xcorr(x, cfg.ninputs, len(chans), cfg.ntime, cfg.dtype)
+    tcal = time.perf_counter() - t0
+    per_chan_span = tcal / len(chans) * min(len(chans), nthreads)  # seconds of one "wave" of nthreads channels
+    waves = max(1, int(target_s / max(per_chan_span * cfg.nspans, 1e-9)))
+    nch = min(cfg.nchan, waves * nthreads)
+    chans = sorted(set(int(round(k * (cfg.nchan - 1) / max(1, nch - 1))) for k in range(nch))) if nch > 1 else [0]
+    slabs = [generate_channel_slab(cfg, s, chans).numpy() for s in range(cfg.nspans)]
+    t0 = time.perf_counter()
+    out = oracle.xcorr(slabs[0], cfg.ninputs, len(chans), cfg.ntime, cfg.dtype)
+    for s in range(1, cfg.nspans):
+        oracle.xcorr(slabs[s], cfg.ninputs, len(chans), cfg.ntime, cfg.dtype, out=out, accumulate=True)
+    dt = time.perf_counter() - t0
+    return dt, len(chans), nthreads
+
+
+def run_reference(args, cfg):
+    """--impl reference: the CPU oracle as the reference arm (there is no reference implementation
+    of this path: /root/reference holds only the paper).  Each step = a bounded channel subset."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    from xcorr_inputs import generate_channel_slab
+    nthreads = oracle.threads()
+    wl = workload_numbers(cfg)
+    nch = min(cfg.nchan, max(1, nthreads))
+    chans = sorted(set(int(round(k * (cfg.nchan - 1) / max(1, nch - 1))) for k in range(nch))) if nch > 1 else [0]
+    slabs = [generate_channel_slab(cfg, s, chans).numpy() for s in range(cfg.nspans)]
+
+    def step():
+        out = oracle.xcorr(slabs[0], cfg.ninputs, len(chans), cfg.ntime, cfg.dtype)
+        for s in range(1, cfg.nspans):
+            oracle.xcorr(slabs[s], cfg.ninputs, len(chans), cfg.ntime, cfg.dtype, out=out, accumulate=True)
+
+    for _ in range(args.warmup):
+        step()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        step()
+    dt = (time.perf_counter() - t0) / args.steps
+    frac = len(chans) / cfg.nchan
+    tops = wl["ops_step"] * frac / dt / 1e12
+    sample = "%d of %d channels (evenly spaced), all %d span(s), full ntime and ninputs, per step" % (
+        len(chans), cfg.nchan, cfg.nspans)
+    line = {"impl": "reference", "metric": METRIC, "value": tops, "unit": "TOPS", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "int8 x int8 -> int32", "data": "synthetic",
+            "config": config_dict(cfg, {"sample": sample}),
+            "samples_per_s": wl["samples_step"] * frac / dt,
+            "cpu_baseline": {"value": tops, "unit": "TOPS", "cores": nthreads, "kind": "oracle", "sample": sample},
+            "e2e": {"value": tops, "unit": "TOPS", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="cfg3", help="cfg1..cfg5 (BASELINE.json configs[0..4])")
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--algo", default="tcgen05", choices=["tcgen05", "simt"])
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
+
+    from xcorr_inputs import CONFIGS, generate_span
+    cfg = CONFIGS[args.config]
+    if args.impl == "reference":
+        run_reference(args, cfg)
+        return
+
+    import torch
+    import paper_1708_00720_b200 as bfx
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the X-engine has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    wl = workload_numbers(cfg)
+    peaks = load_peaks()
+    algo = bfx.BF_XCORR_ALGO_TCGEN05 if args.algo == "tcgen05" else bfx.BF_XCORR_ALGO_SIMT
+
+    # ---- synthetic spans, resident in HBM (every rank holds one full per-GPU workload: a channel shard)
+    spans = [generate_span(cfg, s, device=dev) for s in range(cfg.nspans)]
+    out = torch.empty((cfg.nchan, cfg.nbaselines, 2), dtype=torch.int32, device=dev)
+    plan = bfx.bfXcorrCreate(cfg.ninputs, cfg.nchan, cfg.ntime, cfg.dtype)
+    bfx.bfXcorrSetAlgo(plan, algo)
+    stream = torch.cuda.current_stream()
+    sptr = stream.cuda_stream
+    launches = 0
+
+    def step(record=None):
+        nonlocal launches
+        for s in range(cfg.nspans):
+            if record is not None:
+                e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+            bfx.bfXcorrExecute(plan, spans[s].data_ptr(), out.data_ptr(), s > 0, sptr)
+            launches += bfx.bfXcorrGetLaunchCount(plan)
+            if record is not None:
+                e1.record(stream)
+                record.append((s, e0, e1))
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    launches = 0
+    rec = []
+    t_begin = torch.cuda.Event(enable_timing=True); t_end = torch.cuda.Event(enable_timing=True)
+    t_begin.record(stream)
+    for _ in range(args.steps):
+        step(rec)
+    t_end.record(stream)
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    total_ms = t_begin.elapsed_time(t_end)
+    if dist is not None:
+        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    ms_per_step = total_ms / args.steps
+    per_span_ms = {}
+    for s, e0, e1 in rec:
+        per_span_ms.setdefault(s, []).append(e0.elapsed_time(e1))
+    launch_ms = [sum(v) / len(v) for _, v in sorted(per_span_ms.items())]
+    mean_launch_ms = sum(sum(v) for v in per_span_ms.values()) / max(1, sum(len(v) for v in per_span_ms.values()))
+    timed_launches = launches
+
+    # ---- end to end through the host-buffer entry point
+    e2e = None
+    if not args.no_e2e:
+        try:
+            host_spans = [torch.empty(cfg.span_bytes, dtype=torch.uint8, pin_memory=True) for _ in range(cfg.nspans)]
+            for h, d in zip(host_spans, spans):
+                h.copy_(d.reshape(-1))
+            host_out = torch.empty((cfg.nchan, cfg.nbaselines, 2), dtype=torch.int32, pin_memory=True)
+            torch.cuda.synchronize()
+
+            def e2e_step():
+                for s in range(cfg.nspans):
+                    last = s == cfg.nspans - 1
+                    bfx.bfXcorrExecuteHost(plan, host_spans[s].data_ptr(), out.data_ptr(),
+                                           host_out.data_ptr() if last else 0, s > 0, sptr)
+
+            e2e_step()
+            barrier()
+            a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            for _ in range(args.e2e_steps):
+                e2e_step()
+            b.record(stream)
+            barrier()
+            e_ms = a.elapsed_time(b)
+            if dist is not None:
+                t = torch.tensor([e_ms], dtype=torch.float64, device=dev)
+                dist.all_reduce(t, op=dist.ReduceOp.MAX)
+                e_ms = float(t.item())
+            e_ms /= args.e2e_steps
+            e2e = {"value": wl["ops_step"] * world / (e_ms * 1e-3) / 1e12, "unit": "TOPS",
+                   "h2d_bytes_per_step": int(cfg.span_bytes * cfg.nspans), "d2h_bytes_per_step": int(cfg.out_bytes),
+                   "ms_per_step": e_ms, "steps": args.e2e_steps,
+                   "samples_per_s": wl["samples_step"] * world / (e_ms * 1e-3),
+                   "api": "bfXcorrExecuteHost (pinned host spans in, visibility buffer out after the last span)"}
+            del host_spans, host_out
+        except RuntimeError as ex:  # pinned allocation refused, etc.
+            e2e = {"value": None, "unit": "TOPS", "error": str(ex)[:200]}
+
+    bfx.bfXcorrDestroy(plan)
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    value = wl["ops_step"] * world / (ms_per_step * 1e-3) / 1e12
+    # ---- roofline of the (only) kernel, per launch, averaged over the spans of a step
+    ops_launch = wl["ops_span"]
+    bytes_launch = wl["bytes_step"] / cfg.nspans
+    t_launch = mean_launch_ms * 1e-3
+    long_region = total_ms > 1000.0
+    bf16_peak = peaks["bf16_sustained"] if long_region else peaks["bf16_burst"]
+    int8_peak = 2.0 * bf16_peak  # guide's nominal int8:bf16 dense ratio (4.5 : 2.25 PFLOP/s)
+    tensor = {"bound": "tensor", "achieved": ops_launch / t_launch / 1e12, "peak": int8_peak, "unit": "TOPS"}
+    tensor["frac"] = tensor["achieved"] / tensor["peak"]
+    hbm = {"bound": "hbm", "achieved": bytes_launch / t_launch / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s"}
+    hbm["frac"] = hbm["achieved"] / hbm["peak"]
+    main_r, alt_r = (tensor, hbm) if tensor["frac"] >= hbm["frac"] else (hbm, tensor)
+    roofline = dict(main_r)
+    roofline["traffic"] = None
+    roofline["peak_source"] = "%s (%s; int8 = 2 x bf16 %s)" % (
+        peaks["source"], "MEASURED_PEAKS.json" if peaks["source"] == "measured" else "B200_PROFILING.md fallback",
+        "sustained" if long_region else "burst")
+    roofline["kernel"] = "xcorr_tcgen05_kernel" if args.algo == "tcgen05" else "xcorr_simt_kernel"
+    roofline["launch_ms"] = launch_ms
+    roofline["algorithmic_ops_per_launch"] = ops_launch
+    roofline["algorithmic_bytes_per_launch"] = bytes_launch
+    roofline["other_bound"] = alt_r
+    roofline["frac_of_nominal_int8_4500"] = tensor["achieved"] / 4500.0
+
+    cpu = None
+    if not args.no_cpu_baseline:
+        dt, nch, nthreads = oracle_sample(cfg, args.cpu_seconds)
+        frac = nch / cfg.nchan
+        cpu = {"value": wl["ops_step"] * frac / dt / 1e12, "unit": "TOPS", "cores": nthreads, "kind": "oracle",
+               "sample": "%d of %d channels (evenly spaced), all %d span(s), full ntime and ninputs; %.1f s" % (
+                   nch, cfg.nchan, cfg.nspans, dt),
+               "samples_per_s": wl["samples_step"] * frac / dt}
+
+    line = {"metric": METRIC, "value": value, "unit": "TOPS", "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "int8 x int8 -> int32", "data": "synthetic",
+            "config": config_dict(cfg, {"l2": "inputs_exceed_l2" if cfg.span_bytes * cfg.nspans > 126e6 else
+                                        "inputs_fit_l2 (latency-bound tiny case)",
+                                        "parallelism": "channels sharded, no collective" if world > 1 else "1 gpu",
+                                        "algo": args.algo}),
+            "samples_per_s": wl["samples_step"] * world / (ms_per_step * 1e-3),
+            "clocks": clocks, "e2e": e2e, "gpu_launches": timed_launches, "roofline": roofline,
+            "cpu_baseline": cpu}
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
