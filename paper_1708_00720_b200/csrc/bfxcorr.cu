@@ -38,6 +38,7 @@ struct bfXcorr_impl {
     // S2: lower-triangle tile table (device copy) for the tcgen05 kernel
     TcTile* d_tiles;
     int tiles_per_chan;
+    unsigned long long* d_sched;  // dynamic tile scheduler state, re-armed by the kernel itself
     EncodeTiledFn encode;
     // staging for bfXcorrExecuteHost
     void* d_stage_in;
@@ -125,6 +126,7 @@ int launch_tcgen05(bfXcorr p, const void* in, void* out, int accumulate, cudaStr
     prm.tiles_per_chan = p->tiles_per_chan;
     prm.ntiles = static_cast<long long>(p->tiles_per_chan) * p->nchan;
     prm.accumulate = accumulate ? 1 : 0;
+    prm.sched = p->d_sched;
     const long long want = prm.ntiles < p->num_sms ? prm.ntiles : p->num_sms;
     const dim3 grid(static_cast<unsigned>(want));
     bfx::xcorr_tcgen05_kernel<CI4><<<grid, TcCfg<CI4>::kThreads, TcCfg<CI4>::kSmemBytes, stream>>>(tmap, prm);
@@ -196,6 +198,8 @@ int bfXcorrCreate(bfXcorr* plan, int ninputs, int nchan, int ntime, int dtype)
     p->tiles_per_chan = static_cast<int>(tiles.size());
     e = cudaMalloc(reinterpret_cast<void**>(&p->d_tiles), tiles.size() * sizeof(TcTile));
     if (e == cudaSuccess) e = cudaMemcpy(p->d_tiles, tiles.data(), tiles.size() * sizeof(TcTile), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMalloc(reinterpret_cast<void**>(&p->d_sched), 2 * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMemset(p->d_sched, 0, 2 * sizeof(unsigned long long));
     if (e == cudaSuccess)
         e = cudaFuncSetAttribute(bfx::xcorr_tcgen05_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  TcCfg<false>::kSmemBytes);
@@ -205,6 +209,7 @@ int bfXcorrCreate(bfXcorr* plan, int ninputs, int nchan, int ntime, int dtype)
     if (e != cudaSuccess) {
         const int st = cuda_fail(nullptr, e);
         if (p->d_tiles) cudaFree(p->d_tiles);
+        if (p->d_sched) cudaFree(p->d_sched);
         delete p;
         return st;
     }
@@ -249,6 +254,7 @@ int bfXcorrDestroy(bfXcorr plan)
 {
     if (!valid(plan)) return BF_XCORR_INVALID_HANDLE;
     if (plan->d_tiles) cudaFree(plan->d_tiles);
+    if (plan->d_sched) cudaFree(plan->d_sched);
     if (plan->d_stage_in) cudaFree(plan->d_stage_in);
     plan->magic = 0;
     delete plan;

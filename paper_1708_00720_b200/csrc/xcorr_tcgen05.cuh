@@ -70,7 +70,10 @@ struct TcParams {
     int tiles_per_chan;
     long long ntiles;  // tiles_per_chan * nchan
     int accumulate;
+    unsigned long long* sched;  // [0] next tile to hand out, [1] CTAs finished (self-resetting, see tc_next_tile)
 };
+
+constexpr int TC_RING = 4;  // depth of the per-CTA ring that passes scheduled tile indices between warp roles
 
 // UMMA shared-memory descriptor, MN-major, SWIZZLE_128B:
 //   bits [0,14) start >> 4 | [16,30) LBO >> 4 (pitch between 128-byte m-blocks) |
@@ -93,6 +96,37 @@ __host__ __device__ constexpr uint32_t tc_instr_desc(int m, int n)
            (static_cast<uint32_t>(m >> 4) << 24);
 }
 
+// S2, device side: tiles are handed out in table order (channel-major) by one global counter, so at any
+// moment the CTAs work on a window of ~num_sms consecutive tiles = a few channels whose slabs stay in L2,
+// however unequal the tiles are.  The producer lane fetches an index and publishes it to the other warp
+// roles of its CTA through a small shared-memory ring.
+struct TcRing {
+    uint32_t bar_sfull, bar_sempty, ring_base;
+
+    __device__ __forceinline__ void publish(uint32_t n, long long w) const
+    {
+        const uint32_t slot = n % TC_RING;
+        asm volatile("st.shared.s64 [%0], %1;" ::"r"(ring_base + 8 * slot), "l"(w) : "memory");
+        ptx::mbar_arrive(bar_sfull + 8 * slot);
+    }
+    __device__ __forceinline__ void wait_free(uint32_t n) const
+    {
+        ptx::mbar_wait(bar_sempty + 8 * (n % TC_RING), ((n / TC_RING) & 1) ^ 1);
+    }
+    // WARP: called by a converged warp (lane 0 releases the slot); else by a single lane
+    template <bool WARP>
+    __device__ __forceinline__ long long get(uint32_t n, uint32_t lane) const
+    {
+        const uint32_t slot = n % TC_RING;
+        ptx::mbar_wait(bar_sfull + 8 * slot, (n / TC_RING) & 1);
+        long long w;
+        asm volatile("ld.shared.s64 %0, [%1];" : "=l"(w) : "r"(ring_base + 8 * slot) : "memory");
+        if (WARP) __syncwarp();
+        if (!WARP || lane == 0) ptx::mbar_arrive(bar_sempty + 8 * slot);
+        return w;
+    }
+};
+
 template <bool CI4>
 __global__ void __launch_bounds__(TcCfg<CI4>::kThreads, 1)
 xcorr_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
@@ -114,7 +148,10 @@ xcorr_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
     const uint32_t bar_tempty = bar_tfull + 16;        // [2]  accumulator drained by the epilogue
     const uint32_t bar_rfull = bar_tempty + 16;        // [R]  ci4: raw bytes landed
     const uint32_t bar_rempty = bar_rfull + 8 * R;     // [R]  ci4: raw bytes consumed
-    const uint32_t tmem_slot = bar_rempty + 8 * R;     // 4 bytes: TMEM base address
+    const uint32_t tmem_slot = bar_rempty + 8 * R;     // 4 bytes: TMEM base address (8 reserved)
+    const uint32_t bar_sfull = tmem_slot + 8;          // [TC_RING] scheduled tile index published
+    const uint32_t bar_sempty = bar_sfull + 8 * TC_RING;  // [TC_RING] every consumer role has read it
+    const uint32_t ring_base = bar_sempty + 8 * TC_RING;  // [TC_RING] int64 tile index, -1 = no more work
 
     const int warp = threadIdx.x >> 5;
     const uint32_t lane = ptx::lane_id();
@@ -134,6 +171,10 @@ xcorr_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
                 ptx::mbar_init(bar_rfull + 8 * s, 1);
                 ptx::mbar_init(bar_rempty + 8 * s, 4);
             }
+        for (int s = 0; s < TC_RING; ++s) {
+            ptx::mbar_init(bar_sfull + 8 * s, 1);
+            ptx::mbar_init(bar_sempty + 8 * s, CI4 ? 9 : 5);  // MMA issuer + 4 epilogue warps (+ 4 unpack warps)
+        }
         ptx::fence_barrier_init();
     }
     if (warp == 2) {
@@ -147,14 +188,19 @@ xcorr_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
 
     const int nkb = (p.ntime + TC_KT - 1) / TC_KT;
-    const long long tile_stride = gridDim.x;
+    const TcRing ring{bar_sfull, bar_sempty, ring_base};
 
     if (warp == 0) {
         // ===================== TMA producer (S1 for ci8, first half of S1 for ci4) =====================
         if (lane == 0) {
             uint32_t stage = 0, phase = 0;
             constexpr int NST = CI4 ? R : S;
-            for (long long w = blockIdx.x; w < p.ntiles; w += tile_stride) {
+            for (uint32_t n = 0;; ++n) {
+                ring.wait_free(n);
+                long long w = static_cast<long long>(atomicAdd(p.sched, 1ull));
+                if (w >= p.ntiles) w = -1;
+                ring.publish(n, w);
+                if (w < 0) break;
                 const int c = static_cast<int>(w / p.tiles_per_chan);
                 const TcTile tl = p.tiles[w % p.tiles_per_chan];
                 const int xbytes = CI4 ? 64 : 128;  // bytes of one 64-input block in a span row
@@ -180,8 +226,9 @@ xcorr_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
         // ===================== MMA issuer (S3) =====================
         if (lane == 0) {
             uint32_t stage = 0, phase = 0;
-            uint32_t it = 0;
-            for (long long w = blockIdx.x; w < p.ntiles; w += tile_stride, ++it) {
+            for (uint32_t it = 0;; ++it) {
+                const long long w = ring.get<false>(it, 0);
+                if (w < 0) break;
                 const TcTile tl = p.tiles[w % p.tiles_per_chan];
                 const uint32_t buf = it & 1, bphase = (it >> 1) & 1;
                 const uint32_t idesc = tc_instr_desc(128, 128 * tl.nbox);
@@ -215,8 +262,9 @@ xcorr_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
         const uint32_t stg_warp = stg_base + wq * TC_STG_WARP_BYTES;
         const uint32_t stg_wr = stg_warp + (lane >> 1) * TC_STG_ROW_BYTES;
         const long long nbl = static_cast<long long>(p.ninputs) * (p.ninputs + 1) / 2;
-        uint32_t it = 0;
-        for (long long w = blockIdx.x; w < p.ntiles; w += tile_stride, ++it) {
+        for (uint32_t it = 0;; ++it) {
+            const long long w = ring.get<true>(it, lane);
+            if (w < 0) break;
             const int c = static_cast<int>(w / p.tiles_per_chan);
             const TcTile tl = p.tiles[w % p.tiles_per_chan];
             const uint32_t buf = it & 1, bphase = (it >> 1) & 1;
@@ -313,7 +361,9 @@ xcorr_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
         const int uw = warp - 8;
         const int tid = uw * 32 + static_cast<int>(lane);  // 0..127
         uint32_t rstage = 0, rphase = 0, ostage = 0, ophase = 0;
-        for (long long w = blockIdx.x; w < p.ntiles; w += tile_stride) {
+        for (uint32_t it = 0;; ++it) {
+            const long long w = ring.get<true>(it, lane);
+            if (w < 0) break;
             const TcTile tl = p.tiles[w % p.tiles_per_chan];
             const int first_box = tl.a_alias < 0 ? 0 : 1;
             const int last_box = tl.nbox;  // boxes first_box..last_box inclusive
@@ -367,6 +417,11 @@ xcorr_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
     ptx::tc_fence_before();
     __syncthreads();
     if (warp == 2) ptx::tmem_dealloc<1>(tmem_base, TC_TMEM_COLS);
+    // the last CTA to finish re-arms the scheduler for the next launch (every CTA has drawn its final index)
+    if (threadIdx.x == 0 && atomicAdd(p.sched + 1, 1ull) == gridDim.x - 1) {
+        p.sched[0] = 0;
+        p.sched[1] = 0;
+    }
 }
 
 }  // namespace bfx
