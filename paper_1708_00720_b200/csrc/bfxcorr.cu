@@ -10,6 +10,7 @@
 #include <cuda_runtime.h>
 
 #include "../../include/bfxcorr.h"
+#include "xcorr_relayout.cuh"
 #include "xcorr_simt.cuh"
 #include "xcorr_tcgen05.cuh"
 
@@ -40,6 +41,8 @@ struct bfXcorr_impl {
     int tiles_per_chan;
     unsigned long long* d_sched;  // dynamic tile scheduler state, re-armed by the kernel itself
     EncodeTiledFn encode;
+    // S1: channel-major int8 copy of the span, z[nchan][ntime][2*ninputs] (NULL: operands come from the span itself)
+    uint8_t* d_z;
     // staging for bfXcorrExecuteHost
     void* d_stage_in;
 };
@@ -92,18 +95,38 @@ std::vector<TcTile> build_tiles(int ninputs)
     return tiles;
 }
 
-int make_tensor_map(bfXcorr p, const void* in, CUtensorMap* tmap)
+// Where the tensor-core kernel reads its operands from: the caller's span x[t][c][...] itself (direct), or the
+// plan's channel-major int8 copy z[c][t][...] written by xcorr_relayout_kernel.  Both are addressed with the
+// same coordinates (byte in row, channel, sample); only the strides differ.
+struct OperandSource {
+    const void* base;
+    unsigned long long row;          // bytes per (sample, channel) row
+    unsigned long long chan_stride;  // bytes between channels
+    unsigned long long time_stride;  // bytes between samples
+    bool raw_ci4;                    // rows hold ci4 bytes (unpacked on chip), else int8 (re, im) pairs
+};
+
+OperandSource direct_source(bfXcorr p, const void* in)
 {
-    // span as a 3-D byte tensor, innermost first: (row bytes, nchan, ntime)
     const unsigned long long row = static_cast<unsigned long long>(p->ninputs) * bytes_per_sample(p->dtype);
-    const cuuint64_t dims[3] = {row, static_cast<cuuint64_t>(p->nchan), static_cast<cuuint64_t>(p->ntime)};
-    const cuuint64_t strides[2] = {row, row * static_cast<cuuint64_t>(p->nchan)};
-    const cuuint32_t box[3] = {p->dtype == BF_XCORR_CI4 ? 64u : 128u, 1u, static_cast<cuuint32_t>(bfx::TC_KT)};
+    return OperandSource{in, row, row, row * static_cast<unsigned long long>(p->nchan), p->dtype == BF_XCORR_CI4};
+}
+
+OperandSource relayout_source(bfXcorr p)
+{
+    const unsigned long long row = 2ull * p->ninputs;
+    return OperandSource{p->d_z, row, row * static_cast<unsigned long long>(p->ntime), row, false};
+}
+
+int encode_map(bfXcorr p, CUtensorMap* m, CUtensorMapDataType type, const OperandSource& src, unsigned elem_bytes,
+               unsigned box_elems, CUtensorMapSwizzle swz)
+{
+    const cuuint64_t dims[3] = {src.row / elem_bytes, static_cast<cuuint64_t>(p->nchan), static_cast<cuuint64_t>(p->ntime)};
+    const cuuint64_t strides[2] = {src.chan_stride, src.time_stride};
+    const cuuint32_t box[3] = {box_elems, 1u, static_cast<cuuint32_t>(bfx::TC_KT)};
     const cuuint32_t estr[3] = {1u, 1u, 1u};
-    const CUresult r = p->encode(tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<void*>(in), dims, strides, box, estr,
-                                 CU_TENSOR_MAP_INTERLEAVE_NONE,
-                                 p->dtype == BF_XCORR_CI4 ? CU_TENSOR_MAP_SWIZZLE_NONE : CU_TENSOR_MAP_SWIZZLE_128B,
-                                 CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    const CUresult r = p->encode(m, type, 3, const_cast<void*>(src.base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                 swz, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) {
         p->last_cuda_error = static_cast<int>(cudaErrorInvalidValue);
         return BF_XCORR_DEVICE_ERROR;
@@ -112,10 +135,18 @@ int make_tensor_map(bfXcorr p, const void* in, CUtensorMap* tmap)
 }
 
 template <bool CI4>
-int launch_tcgen05(bfXcorr p, const void* in, void* out, int accumulate, cudaStream_t stream)
+int launch_tcgen05(bfXcorr p, const OperandSource& src, void* out, int accumulate, cudaStream_t stream)
 {
-    CUtensorMap tmap;
-    const int st = make_tensor_map(p, in, &tmap);
+    CUtensorMap tmap, pmap;
+    // operand boxes: 64 inputs x 1 channel x TC_KT samples (128 bytes of int8 pairs, or 64 raw ci4 bytes)
+    int st = encode_map(p, &tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, src, 1, CI4 ? 64u : 128u,
+                        CI4 ? CU_TENSOR_MAP_SWIZZLE_NONE : CU_TENSOR_MAP_SWIZZLE_128B);
+    if (st != BF_XCORR_OK) return st;
+    // whole rows as 32-bit words, for L2 prefetch only: boxes of up to 256 words x TC_KT samples
+    const unsigned long long words = src.row / 4;
+    const int pf_bx = static_cast<int>(words < 256 ? words : 256);
+    const int pf_nx = static_cast<int>((words + pf_bx - 1) / pf_bx);
+    st = encode_map(p, &pmap, CU_TENSOR_MAP_DATA_TYPE_UINT32, src, 4, static_cast<unsigned>(pf_bx), CU_TENSOR_MAP_SWIZZLE_NONE);
     if (st != BF_XCORR_OK) return st;
     TcParams prm;
     prm.out = static_cast<int32_t*>(out);
@@ -129,10 +160,31 @@ int launch_tcgen05(bfXcorr p, const void* in, void* out, int accumulate, cudaStr
     prm.sched = p->d_sched;
     const long long want = prm.ntiles < p->num_sms ? prm.ntiles : p->num_sms;
     const dim3 grid(static_cast<unsigned>(want));
-    bfx::xcorr_tcgen05_kernel<CI4><<<grid, TcCfg<CI4>::kThreads, TcCfg<CI4>::kSmemBytes, stream>>>(tmap, prm);
+    // the CTAs work on a window of `grid` consecutive tiles = grid / tiles_per_chan channels; prefetch past it
+    prm.pf_dist = static_cast<int>(want / p->tiles_per_chan) + 2;
+    prm.pf_nx = pf_nx;
+    prm.pf_bx = pf_bx;
+    bfx::xcorr_tcgen05_kernel<CI4><<<grid, TcCfg<CI4>::kThreads, TcCfg<CI4>::kSmemBytes, stream>>>(tmap, pmap, prm);
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(p, e);
-    p->last_launch_count = 1;
+    p->last_launch_count += 1;
+    return BF_XCORR_OK;
+}
+
+// S1 as its own pass (xcorr_relayout.cuh): span -> channel-major int8 copy owned by the plan
+int launch_relayout(bfXcorr p, const void* in, cudaStream_t stream)
+{
+    const int row_in = static_cast<int>(p->ninputs * bytes_per_sample(p->dtype));
+    const dim3 grid(static_cast<unsigned>((p->ntime + bfx::RL_TB - 1) / bfx::RL_TB), static_cast<unsigned>(p->nchan));
+    if (p->dtype == BF_XCORR_CI4)
+        bfx::xcorr_relayout_kernel<true><<<grid, bfx::RL_THREADS, 0, stream>>>(static_cast<const uint8_t*>(in), p->d_z, row_in,
+                                                                               p->nchan, p->ntime);
+    else
+        bfx::xcorr_relayout_kernel<false><<<grid, bfx::RL_THREADS, 0, stream>>>(static_cast<const uint8_t*>(in), p->d_z, row_in,
+                                                                                p->nchan, p->ntime);
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(p, e);
+    p->last_launch_count += 1;
     return BF_XCORR_OK;
 }
 
@@ -144,7 +196,7 @@ int launch_simt(bfXcorr p, const void* in, void* out, int accumulate, cudaStream
                                                      p->ninputs, p->nchan, p->ntime, p->dtype, accumulate ? 1 : 0);
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(p, e);
-    p->last_launch_count = 1;
+    p->last_launch_count += 1;
     return BF_XCORR_OK;
 }
 
@@ -200,6 +252,10 @@ int bfXcorrCreate(bfXcorr* plan, int ninputs, int nchan, int ntime, int dtype)
     if (e == cudaSuccess) e = cudaMemcpy(p->d_tiles, tiles.data(), tiles.size() * sizeof(TcTile), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMalloc(reinterpret_cast<void**>(&p->d_sched), 2 * sizeof(unsigned long long));
     if (e == cudaSuccess) e = cudaMemset(p->d_sched, 0, 2 * sizeof(unsigned long long));
+    // A channel whose tiles re-read its samples is first rewritten channel-major (xcorr_relayout.cuh); with a
+    // single tile per channel (ninputs <= 64) every sample is read once anyway and the span is used in place.
+    if (e == cudaSuccess && p->tiles_per_chan > 1)
+        e = cudaMalloc(reinterpret_cast<void**>(&p->d_z), static_cast<size_t>(ntime) * nchan * ninputs * 2ull);
     if (e == cudaSuccess)
         e = cudaFuncSetAttribute(bfx::xcorr_tcgen05_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  TcCfg<false>::kSmemBytes);
@@ -210,6 +266,7 @@ int bfXcorrCreate(bfXcorr* plan, int ninputs, int nchan, int ntime, int dtype)
         const int st = cuda_fail(nullptr, e);
         if (p->d_tiles) cudaFree(p->d_tiles);
         if (p->d_sched) cudaFree(p->d_sched);
+        if (p->d_z) cudaFree(p->d_z);
         delete p;
         return st;
     }
@@ -225,8 +282,13 @@ int bfXcorrExecute(bfXcorr plan, const void* in, void* out, int accumulate, void
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     plan->last_launch_count = 0;
     if (plan->algo == BF_XCORR_ALGO_SIMT) return launch_simt(plan, in, out, accumulate, s);
-    return plan->dtype == BF_XCORR_CI4 ? launch_tcgen05<true>(plan, in, out, accumulate, s)
-                                       : launch_tcgen05<false>(plan, in, out, accumulate, s);
+    if (plan->d_z) {
+        const int st = launch_relayout(plan, in, s);
+        if (st != BF_XCORR_OK) return st;
+        return launch_tcgen05<false>(plan, relayout_source(plan), out, accumulate, s);
+    }
+    return plan->dtype == BF_XCORR_CI4 ? launch_tcgen05<true>(plan, direct_source(plan, in), out, accumulate, s)
+                                       : launch_tcgen05<false>(plan, direct_source(plan, in), out, accumulate, s);
 }
 
 int bfXcorrExecuteHost(bfXcorr plan, const void* in_host, void* out_dev, void* out_host, int accumulate, void* stream)
@@ -256,6 +318,7 @@ int bfXcorrDestroy(bfXcorr plan)
     if (plan->d_tiles) cudaFree(plan->d_tiles);
     if (plan->d_sched) cudaFree(plan->d_sched);
     if (plan->d_stage_in) cudaFree(plan->d_stage_in);
+    if (plan->d_z) cudaFree(plan->d_z);
     plan->magic = 0;
     delete plan;
     return BF_XCORR_OK;

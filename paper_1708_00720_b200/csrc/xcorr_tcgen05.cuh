@@ -40,8 +40,9 @@ constexpr int TC_STAGE_BYTES = 3 * TC_BOX_BYTES; // A, B0, B1
 constexpr int TC_RAW_BOX_BYTES = TC_KT * 64;     // ci4: one raw box, KT rows of 64 bytes
 constexpr int TC_RAW_STAGE_BYTES = 3 * TC_RAW_BOX_BYTES;
 constexpr int TC_CJ = 64;                        // visibilities (columns j) per epilogue chunk
-constexpr int TC_STG_ROW_BYTES = TC_CJ * 8 + 16; // staging row pitch, +16 B keeps 8 rows on distinct banks
-constexpr int TC_STG_WARP_BYTES = 16 * TC_STG_ROW_BYTES;
+constexpr int TC_STG_PITCH = TC_CJ * 8 + 8;      // staging row pitch: 130 words -> 16 rows hit 16 distinct bank pairs
+constexpr int TC_STG_BUF_BYTES = 16 * TC_STG_PITCH;   // one warp's 16 rows x 64 visibilities
+constexpr int TC_STG_WARP_BYTES = 2 * TC_STG_BUF_BYTES;  // double buffered against the asynchronous bulk copies
 constexpr int TC_STG_BYTES = 4 * TC_STG_WARP_BYTES;
 constexpr int TC_TMEM_COLS = 512;                // two 256-column accumulators
 
@@ -71,6 +72,9 @@ struct TcParams {
     long long ntiles;  // tiles_per_chan * nchan
     int accumulate;
     unsigned long long* sched;  // [0] next tile to hand out, [1] CTAs finished (self-resetting, see tc_next_tile)
+    // L2 prefetch of the span rows of a channel `pf_dist` channels ahead of the one being worked on
+    // (pmap: whole rows, boxes of pf_bx 32-bit words x TC_KT samples; pf_nx boxes cover one row)
+    int pf_dist, pf_nx, pf_bx;
 };
 
 constexpr int TC_RING = 4;  // depth of the per-CTA ring that passes scheduled tile indices between warp roles
@@ -129,7 +133,7 @@ struct TcRing {
 
 template <bool CI4>
 __global__ void __launch_bounds__(TcCfg<CI4>::kThreads, 1)
-xcorr_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
+xcorr_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ CUtensorMap pmap, const TcParams p)
 {
     using Cfg = TcCfg<CI4>;
     constexpr int S = Cfg::kOpStages;
@@ -158,6 +162,7 @@ xcorr_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
 
     if (warp == 0 && lane == 0) {
         ptx::prefetch_tensormap(&tmap);
+        ptx::prefetch_tensormap(&pmap);
         for (int s = 0; s < S; ++s) {
             ptx::mbar_init(bar_full + 8 * s, CI4 ? 4 : 1);
             ptx::mbar_init(bar_empty + 8 * s, 1);
@@ -202,7 +207,17 @@ xcorr_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
                 ring.publish(n, w);
                 if (w < 0) break;
                 const int c = static_cast<int>(w / p.tiles_per_chan);
-                const TcTile tl = p.tiles[w % p.tiles_per_chan];
+                const int q = static_cast<int>(w % p.tiles_per_chan);
+                const TcTile tl = p.tiles[q];
+                // The operand boxes are 64..128-byte pieces of rows that lie nchan*row bytes apart: fetched on
+                // demand they reach DRAM as scattered short bursts and every TMA load waits a DRAM latency.
+                // So the tiles of channel c share out the job of pulling channel c + pf_dist into the L2 as
+                // whole rows, and the operand loads further down become L2 hits.
+                if (c + p.pf_dist < p.nchan) {
+                    const int units = nkb * p.pf_nx;
+                    for (int u = q; u < units; u += p.tiles_per_chan)
+                        ptx::tma_prefetch_l2_3d(&pmap, (u % p.pf_nx) * p.pf_bx, c + p.pf_dist, (u / p.pf_nx) * TC_KT);
+                }
                 const int xbytes = CI4 ? 64 : 128;  // bytes of one 64-input block in a span row
                 const int xa = tl.row_blk * xbytes;
                 const int xb = tl.col_blk * 2 * xbytes;
@@ -256,12 +271,24 @@ xcorr_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
         }
     } else if (warp >= 4 && warp < 8) {
         // ===================== epilogue (S4) =====================
+        // TMEM lane = real row m = 2 i + part of the A block, so lanes (2k, 2k+1) hold the re and im rows of
+        // input row k of this warp.  One shuffle per column pair forms Re V (even lane) / Im V (odd lane);
+        // both lanes store their 4-byte half of the visibility into a per-warp staging row (conflict free:
+        // pitch = 130 words).  Lanes 0..15 then each own one packed-triangle row segment of <= 64
+        // visibilities and hand it to the TMA unit: a bulk store (accumulate = 0) or a bulk int32
+        // reduce-add performed at the L2 (accumulate != 0), so the old values never travel to the SM.
+        // Bulk copies need 16-byte alignment but triangle rows are only 8-byte aligned: a staging row is
+        // placed in a slot of the same address parity as its global start (rows i = 1, 2 mod 4 start on
+        // an odd visibility) and an odd head / tail visibility goes out as a scalar store / red.
         const int wq = warp - 4;                      // TMEM lane quarter
         const uint32_t par = lane & 1;                // 0: re row of its input, 1: im row
         const int sgn = par ? -1 : 1;
+        const uint32_t krow = lane >> 1;
         const uint32_t stg_warp = stg_base + wq * TC_STG_WARP_BYTES;
-        const uint32_t stg_wr = stg_warp + (lane >> 1) * TC_STG_ROW_BYTES;
+        const uint32_t wr_off = (krow ^ ((krow >> 1) & 1)) * TC_STG_PITCH + 4 * par;
+        const uint32_t own_off = (lane ^ ((lane >> 1) & 1)) * TC_STG_PITCH;  // lanes 0..15: slot of row `lane`
         const long long nbl = static_cast<long long>(p.ninputs) * (p.ninputs + 1) / 2;
+        uint32_t nchunks_done = 0;
         for (uint32_t it = 0;; ++it) {
             const long long w = ring.get<true>(it, lane);
             if (w < 0) break;
@@ -272,33 +299,30 @@ xcorr_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
             const int j0 = tl.col_blk * TC_BN_IN;
             const int nchunk = tl.nbox;                       // 64 visibilities columns per chunk
             int32_t* const out_c = p.out + 2 * (static_cast<long long>(c) * nbl);
+            const int i_own = i0 + static_cast<int>(lane);    // lanes 0..15
+            const long long rowk_own = static_cast<long long>(i_own) * (i_own + 1) / 2;
 
             ptx::mbar_wait(bar_tfull + 8 * buf, bphase);
             ptx::tc_fence_after();
-            for (int jc = 0; jc < nchunk; ++jc) {
+            for (int jc = 0; jc < nchunk; ++jc, ++nchunks_done) {
+                const uint32_t stg_buf = stg_warp + (nchunks_done & 1) * TC_STG_BUF_BYTES;
+                // the bulk group that read this staging buffer two chunks ago must be done with it
+                if (lane < 16) ptx::bulk_wait_read<1>();
+                __syncwarp();
                 const uint32_t tcol = tmem_base + (static_cast<uint32_t>(32 * wq) << 16) + buf * 256 + jc * 128;
-#pragma unroll 1
+#pragma unroll
                 for (int q = 0; q < 4; ++q) {
                     uint32_t g[32];
                     ptx::tmem_ld_32x32b_x32(tcol + q * 32, g);
                     ptx::tmem_ld_wait();
-                    int val[16];
 #pragma unroll
                     for (int k = 0; k < 16; ++k) {
                         int ge = static_cast<int>(g[2 * k]), go = static_cast<int>(g[2 * k + 1]);
                         if (CI4) { ge >>= 8; go >>= 8; }       // G came out scaled by 16*16, exactly
                         const int v = __shfl_xor_sync(0xffffffffu, go, 1);
-                        val[k] = ge + sgn * v;                 // even lane: Re V[i][j_k]; odd lane: Im V[i][j_k]
-                    }
-#pragma unroll
-                    for (int kk = 0; kk < 8; ++kk) {
-                        const int send = par ? val[2 * kk] : val[2 * kk + 1];
-                        const int recv = __shfl_xor_sync(0xffffffffu, send, 1);
-                        // even lane keeps j = 2kk (re own, im received); odd lane keeps j = 2kk+1
-                        const int re = par ? recv : val[2 * kk];
-                        const int im = par ? val[2 * kk + 1] : recv;
-                        const uint32_t a = stg_wr + (q * 16 + 2 * kk + par) * 8;
-                        asm volatile("st.shared.v2.s32 [%0], {%1, %2};" ::"r"(a), "r"(re), "r"(im) : "memory");
+                        // even lane: Re V[i][j] = G[2i][2j] + G[2i+1][2j+1]; odd lane: Im V[i][j] = G[2i+1][2j] - G[2i][2j+1]
+                        const int val = ge + sgn * v;
+                        asm volatile("st.shared.s32 [%0], %1;" ::"r"(stg_buf + wr_off + (q * 16 + k) * 8), "r"(val) : "memory");
                     }
                 }
                 if (jc == nchunk - 1) {
@@ -307,52 +331,39 @@ xcorr_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
                     __syncwarp();
                     if (lane == 0) ptx::mbar_arrive(bar_tempty + 8 * buf);
                 }
+                ptx::fence_proxy_async_smem();  // staging writes -> visible to the bulk-copy engine
                 __syncwarp();
-                // coalesced write-out of this warp's 16 rows x 64 columns
-                const int jb = j0 + jc * TC_CJ;
-#pragma unroll 1
-                for (int rg = 0; rg < 16; rg += 4) {
-                    int2 acc[4][2];
-                    int2 old[4][2];
-                    bool ok[4][2];
-#pragma unroll
-                    for (int r = 0; r < 4; ++r) {
-                        const int i = i0 + rg + r;
-                        const long long rowk = static_cast<long long>(i) * (i + 1) / 2;
-#pragma unroll
-                        for (int h = 0; h < 2; ++h) {
-                            const int j = jb + 32 * h + static_cast<int>(lane);
-                            ok[r][h] = (i < p.ninputs) && (j <= i);
-                            old[r][h] = make_int2(0, 0);
-                            if (ok[r][h] && p.accumulate) old[r][h] = ptx::ld_global_v2(out_c + 2 * (rowk + j));
+                if (lane < 16) {
+                    const int jb = j0 + jc * TC_CJ;
+                    int n = i_own + 1 - jb;       // row i holds columns j <= i only (S2 masking of diagonal tiles)
+                    n = n > TC_CJ ? TC_CJ : n;
+                    if (i_own >= p.ninputs) n = 0;
+                    if (n > 0) {
+                        const long long e0 = rowk_own + jb;
+                        int32_t* const g0 = out_c + 2 * e0;
+                        const uint32_t s0 = stg_buf + own_off;
+                        const int head = static_cast<int>(e0 & 1);
+                        const int nbulk = (n - head) & ~1;
+                        if (head) {
+                            int2 v;
+                            asm volatile("ld.shared.v2.s32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(s0));
+                            if (p.accumulate) ptx::red_add_global_v2(g0, v); else ptx::st_global_v2(g0, v);
+                        }
+                        if (nbulk > 0) {
+                            if (p.accumulate) ptx::bulk_reduce_add_s32(g0 + 2 * head, s0 + 8 * head, 8u * nbulk);
+                            else ptx::bulk_store(g0 + 2 * head, s0 + 8 * head, 8u * nbulk);
+                        }
+                        if (head + nbulk < n) {
+                            int2 v;
+                            asm volatile("ld.shared.v2.s32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(s0 + 8 * (n - 1)));
+                            if (p.accumulate) ptx::red_add_global_v2(g0 + 2 * (n - 1), v); else ptx::st_global_v2(g0 + 2 * (n - 1), v);
                         }
                     }
-#pragma unroll
-                    for (int r = 0; r < 4; ++r)
-#pragma unroll
-                        for (int h = 0; h < 2; ++h) {
-                            const uint32_t a = stg_warp + (rg + r) * TC_STG_ROW_BYTES + (32 * h + lane) * 8;
-                            asm volatile("ld.shared.v2.s32 {%0, %1}, [%2];" : "=r"(acc[r][h].x), "=r"(acc[r][h].y) : "r"(a));
-                        }
-#pragma unroll
-                    for (int r = 0; r < 4; ++r) {
-                        const int i = i0 + rg + r;
-                        const long long rowk = static_cast<long long>(i) * (i + 1) / 2;
-#pragma unroll
-                        for (int h = 0; h < 2; ++h) {
-                            const int j = jb + 32 * h + static_cast<int>(lane);
-                            if (ok[r][h]) {
-                                int2 v;
-                                v.x = static_cast<int>(static_cast<uint32_t>(acc[r][h].x) + static_cast<uint32_t>(old[r][h].x));
-                                v.y = static_cast<int>(static_cast<uint32_t>(acc[r][h].y) + static_cast<uint32_t>(old[r][h].y));
-                                ptx::st_global_v2(out_c + 2 * (rowk + j), v);
-                            }
-                        }
-                    }
+                    ptx::bulk_commit();
                 }
-                __syncwarp();
             }
         }
+        if (lane < 16) ptx::bulk_wait_read<0>();  // shared memory must outlive the bulk reads
     } else if (CI4 && warp >= 8) {
         // ===================== ci4 unpack warps (second half of S1) =====================
         // raw stage: 3 boxes [KT][64 B] (one byte per sample: re<<4 | im&15, include/bfxcorr.h)
