@@ -10,7 +10,6 @@
 #include <cuda_runtime.h>
 
 #include "../../include/bfxcorr.h"
-#include "xcorr_relayout.cuh"
 #include "xcorr_simt.cuh"
 #include "xcorr_tcgen05.cuh"
 
@@ -41,8 +40,12 @@ struct bfXcorr_impl {
     int tiles_per_chan;
     unsigned long long* d_sched;  // dynamic tile scheduler state, re-armed by the kernel itself
     EncodeTiledFn encode;
-    // S1: channel-major int8 copy of the span, z[nchan][ntime][2*ninputs] (NULL: operands come from the span itself)
+    // S1: ring of ring_w channel slabs z[c % ring_w][ntime][2*ninputs] int8, filled ahead of the
+    // contraction by the relayout warps of the same kernel (NULL: operands come from the span itself)
     uint8_t* d_z;
+    int ring_w;
+    unsigned long long* d_flags;  // ready[nchan], done[nchan]
+    unsigned long long epoch;     // fused launches so far
     // staging for bfXcorrExecuteHost
     void* d_stage_in;
 };
@@ -112,16 +115,16 @@ OperandSource direct_source(bfXcorr p, const void* in)
     return OperandSource{in, row, row, row * static_cast<unsigned long long>(p->nchan), p->dtype == BF_XCORR_CI4};
 }
 
-OperandSource relayout_source(bfXcorr p)
+OperandSource ring_source(bfXcorr p)
 {
     const unsigned long long row = 2ull * p->ninputs;
     return OperandSource{p->d_z, row, row * static_cast<unsigned long long>(p->ntime), row, false};
 }
 
 int encode_map(bfXcorr p, CUtensorMap* m, CUtensorMapDataType type, const OperandSource& src, unsigned elem_bytes,
-               unsigned box_elems, CUtensorMapSwizzle swz)
+               unsigned box_elems, CUtensorMapSwizzle swz, int nchan_src)
 {
-    const cuuint64_t dims[3] = {src.row / elem_bytes, static_cast<cuuint64_t>(p->nchan), static_cast<cuuint64_t>(p->ntime)};
+    const cuuint64_t dims[3] = {src.row / elem_bytes, static_cast<cuuint64_t>(nchan_src), static_cast<cuuint64_t>(p->ntime)};
     const cuuint64_t strides[2] = {src.chan_stride, src.time_stride};
     const cuuint32_t box[3] = {box_elems, 1u, static_cast<cuuint32_t>(bfx::TC_KT)};
     const cuuint32_t estr[3] = {1u, 1u, 1u};
@@ -135,20 +138,17 @@ int encode_map(bfXcorr p, CUtensorMap* m, CUtensorMapDataType type, const Operan
 }
 
 template <bool CI4>
-int launch_tcgen05(bfXcorr p, const OperandSource& src, void* out, int accumulate, cudaStream_t stream)
+int launch_tcgen05(bfXcorr p, const void* in, void* out, int accumulate, cudaStream_t stream)
 {
-    CUtensorMap tmap, pmap;
+    const bool fused = p->d_z != nullptr;
+    const OperandSource src = fused ? ring_source(p) : direct_source(p, in);
+    CUtensorMap tmap;
     // operand boxes: 64 inputs x 1 channel x TC_KT samples (128 bytes of int8 pairs, or 64 raw ci4 bytes)
-    int st = encode_map(p, &tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, src, 1, CI4 ? 64u : 128u,
-                        CI4 ? CU_TENSOR_MAP_SWIZZLE_NONE : CU_TENSOR_MAP_SWIZZLE_128B);
-    if (st != BF_XCORR_OK) return st;
-    // whole rows as 32-bit words, for L2 prefetch only: boxes of up to 256 words x TC_KT samples
-    const unsigned long long words = src.row / 4;
-    const int pf_bx = static_cast<int>(words < 256 ? words : 256);
-    const int pf_nx = static_cast<int>((words + pf_bx - 1) / pf_bx);
-    st = encode_map(p, &pmap, CU_TENSOR_MAP_DATA_TYPE_UINT32, src, 4, static_cast<unsigned>(pf_bx), CU_TENSOR_MAP_SWIZZLE_NONE);
+    const int st = encode_map(p, &tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, src, 1, CI4 ? 64u : 128u,
+                              CI4 ? CU_TENSOR_MAP_SWIZZLE_NONE : CU_TENSOR_MAP_SWIZZLE_128B, fused ? p->ring_w : p->nchan);
     if (st != BF_XCORR_OK) return st;
     TcParams prm;
+    std::memset(&prm, 0, sizeof(prm));
     prm.out = static_cast<int32_t*>(out);
     prm.tiles = p->d_tiles;
     prm.ninputs = p->ninputs;
@@ -158,30 +158,22 @@ int launch_tcgen05(bfXcorr p, const OperandSource& src, void* out, int accumulat
     prm.ntiles = static_cast<long long>(p->tiles_per_chan) * p->nchan;
     prm.accumulate = accumulate ? 1 : 0;
     prm.sched = p->d_sched;
+    if (fused) {
+        prm.rl_enabled = 1;
+        prm.rl_ci4 = p->dtype == BF_XCORR_CI4 ? 1 : 0;
+        prm.x = static_cast<const uint8_t*>(in);
+        prm.z = p->d_z;
+        prm.row_in = static_cast<int>(p->ninputs * bytes_per_sample(p->dtype));
+        prm.ring_w = p->ring_w;
+        prm.rl_nx = (prm.row_in + bfx::RL_XBYTES - 1) / bfx::RL_XBYTES;
+        prm.rl_units = prm.rl_nx * ((p->ntime + bfx::RL_ROWS - 1) / bfx::RL_ROWS);
+        prm.ready = p->d_flags;
+        prm.done = p->d_flags + p->nchan;
+        prm.epoch = ++p->epoch;
+    }
     const long long want = prm.ntiles < p->num_sms ? prm.ntiles : p->num_sms;
     const dim3 grid(static_cast<unsigned>(want));
-    // the CTAs work on a window of `grid` consecutive tiles = grid / tiles_per_chan channels; prefetch past it
-    prm.pf_dist = static_cast<int>(want / p->tiles_per_chan) + 2;
-    prm.pf_nx = pf_nx;
-    prm.pf_bx = pf_bx;
-    bfx::xcorr_tcgen05_kernel<CI4><<<grid, TcCfg<CI4>::kThreads, TcCfg<CI4>::kSmemBytes, stream>>>(tmap, pmap, prm);
-    const cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) return cuda_fail(p, e);
-    p->last_launch_count += 1;
-    return BF_XCORR_OK;
-}
-
-// S1 as its own pass (xcorr_relayout.cuh): span -> channel-major int8 copy owned by the plan
-int launch_relayout(bfXcorr p, const void* in, cudaStream_t stream)
-{
-    const int row_in = static_cast<int>(p->ninputs * bytes_per_sample(p->dtype));
-    const dim3 grid(static_cast<unsigned>((p->ntime + bfx::RL_TB - 1) / bfx::RL_TB), static_cast<unsigned>(p->nchan));
-    if (p->dtype == BF_XCORR_CI4)
-        bfx::xcorr_relayout_kernel<true><<<grid, bfx::RL_THREADS, 0, stream>>>(static_cast<const uint8_t*>(in), p->d_z, row_in,
-                                                                               p->nchan, p->ntime);
-    else
-        bfx::xcorr_relayout_kernel<false><<<grid, bfx::RL_THREADS, 0, stream>>>(static_cast<const uint8_t*>(in), p->d_z, row_in,
-                                                                                p->nchan, p->ntime);
+    bfx::xcorr_tcgen05_kernel<CI4><<<grid, TcCfg<CI4>::kThreads, TcCfg<CI4>::kSmemBytes, stream>>>(tmap, prm);
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(p, e);
     p->last_launch_count += 1;
@@ -250,12 +242,25 @@ int bfXcorrCreate(bfXcorr* plan, int ninputs, int nchan, int ntime, int dtype)
     p->tiles_per_chan = static_cast<int>(tiles.size());
     e = cudaMalloc(reinterpret_cast<void**>(&p->d_tiles), tiles.size() * sizeof(TcTile));
     if (e == cudaSuccess) e = cudaMemcpy(p->d_tiles, tiles.data(), tiles.size() * sizeof(TcTile), cudaMemcpyHostToDevice);
-    if (e == cudaSuccess) e = cudaMalloc(reinterpret_cast<void**>(&p->d_sched), 2 * sizeof(unsigned long long));
-    if (e == cudaSuccess) e = cudaMemset(p->d_sched, 0, 2 * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMalloc(reinterpret_cast<void**>(&p->d_sched), 4 * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMemset(p->d_sched, 0, 4 * sizeof(unsigned long long));
     // A channel whose tiles re-read its samples is first rewritten channel-major (xcorr_relayout.cuh); with a
     // single tile per channel (ninputs <= 64) every sample is read once anyway and the span is used in place.
-    if (e == cudaSuccess && p->tiles_per_chan > 1)
-        e = cudaMalloc(reinterpret_cast<void**>(&p->d_z), static_cast<size_t>(ntime) * nchan * ninputs * 2ull);
+    if (e == cudaSuccess && p->tiles_per_chan > 1) {
+        // window = channels the grid works on at once (doubled: producers run a tile or two ahead of their loads);
+        // on top of that the ring holds ~16 MiB of look-ahead, so a slab is complete long before its first tile is
+        // drawn and stays L2-resident until its last tile is done
+        const unsigned long long slab = static_cast<unsigned long long>(ntime) * ninputs * 2ull;
+        const int window = (p->num_sms + p->tiles_per_chan - 1) / p->tiles_per_chan;
+        long long ahead = static_cast<long long>((16ull << 20) / slab);
+        if (ahead < 2) ahead = 2;
+        long long ring = 2 * window + 2 + ahead;
+        if (ring > nchan) ring = nchan;
+        p->ring_w = static_cast<int>(ring);
+        e = cudaMalloc(reinterpret_cast<void**>(&p->d_z), static_cast<size_t>(ring) * slab);
+        if (e == cudaSuccess) e = cudaMalloc(reinterpret_cast<void**>(&p->d_flags), 2ull * nchan * sizeof(unsigned long long));
+        if (e == cudaSuccess) e = cudaMemset(p->d_flags, 0, 2ull * nchan * sizeof(unsigned long long));
+    }
     if (e == cudaSuccess)
         e = cudaFuncSetAttribute(bfx::xcorr_tcgen05_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  TcCfg<false>::kSmemBytes);
@@ -267,6 +272,7 @@ int bfXcorrCreate(bfXcorr* plan, int ninputs, int nchan, int ntime, int dtype)
         if (p->d_tiles) cudaFree(p->d_tiles);
         if (p->d_sched) cudaFree(p->d_sched);
         if (p->d_z) cudaFree(p->d_z);
+        if (p->d_flags) cudaFree(p->d_flags);
         delete p;
         return st;
     }
@@ -282,13 +288,9 @@ int bfXcorrExecute(bfXcorr plan, const void* in, void* out, int accumulate, void
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     plan->last_launch_count = 0;
     if (plan->algo == BF_XCORR_ALGO_SIMT) return launch_simt(plan, in, out, accumulate, s);
-    if (plan->d_z) {
-        const int st = launch_relayout(plan, in, s);
-        if (st != BF_XCORR_OK) return st;
-        return launch_tcgen05<false>(plan, relayout_source(plan), out, accumulate, s);
-    }
-    return plan->dtype == BF_XCORR_CI4 ? launch_tcgen05<true>(plan, direct_source(plan, in), out, accumulate, s)
-                                       : launch_tcgen05<false>(plan, direct_source(plan, in), out, accumulate, s);
+    if (plan->d_z) return launch_tcgen05<false>(plan, in, out, accumulate, s);  // S1 fused: dtype handled by the relayout warps
+    return plan->dtype == BF_XCORR_CI4 ? launch_tcgen05<true>(plan, in, out, accumulate, s)
+                                       : launch_tcgen05<false>(plan, in, out, accumulate, s);
 }
 
 int bfXcorrExecuteHost(bfXcorr plan, const void* in_host, void* out_dev, void* out_host, int accumulate, void* stream)
@@ -319,6 +321,7 @@ int bfXcorrDestroy(bfXcorr plan)
     if (plan->d_sched) cudaFree(plan->d_sched);
     if (plan->d_stage_in) cudaFree(plan->d_stage_in);
     if (plan->d_z) cudaFree(plan->d_z);
+    if (plan->d_flags) cudaFree(plan->d_flags);
     plan->magic = 0;
     delete plan;
     return BF_XCORR_OK;

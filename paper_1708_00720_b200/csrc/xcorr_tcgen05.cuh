@@ -50,7 +50,7 @@ template <bool CI4>
 struct TcCfg {
     static constexpr int kOpStages = CI4 ? 4 : 6;   // int8 operand ring the MMA reads
     static constexpr int kRawStages = CI4 ? 4 : 0;  // ci4: raw byte ring the TMA fills
-    static constexpr int kThreads = CI4 ? 384 : 256;
+    static constexpr int kThreads = CI4 ? 384 : 512;  // direct ci4: 4 unpack warps; else up to 8 relayout warps
     static constexpr int kSmemBytes = 1024 /*align slack*/ + kOpStages * TC_STAGE_BYTES +
                                       kRawStages * TC_RAW_STAGE_BYTES + TC_STG_BYTES + 512 /*barriers*/;
 };
@@ -72,10 +72,24 @@ struct TcParams {
     long long ntiles;  // tiles_per_chan * nchan
     int accumulate;
     unsigned long long* sched;  // [0] next tile to hand out, [1] CTAs finished (self-resetting, see tc_next_tile)
-    // L2 prefetch of the span rows of a channel `pf_dist` channels ahead of the one being worked on
-    // (pmap: whole rows, boxes of pf_bx 32-bit words x TC_KT samples; pf_nx boxes cover one row)
-    int pf_dist, pf_nx, pf_bx;
+    // ---- S1 fused into this kernel (rl_enabled): the operands are read from a ring `z` of ring_w channel
+    // slabs, z[c % ring_w][t][2 i + part] int8, that the relayout warps fill from the span `x`
+    // ahead of the tiles being contracted.  ready[c] / done[c] count, over all launches of the
+    // plan, the relayout units written for channel c / the tiles of channel c whose loads have landed.
+    int rl_enabled, rl_ci4;
+    const uint8_t* x;
+    uint8_t* z;
+    int row_in;             // bytes of one (t, c) row of the span
+    int ring_w;
+    int rl_nx, rl_units;    // 1 KiB pieces per row; relayout units per channel = rl_nx * ceil(ntime / RL_ROWS)
+    unsigned long long* ready;
+    unsigned long long* done;
+    unsigned long long epoch;  // 1, 2, ... : launch number of this plan
 };
+
+constexpr int RL_ROWS = 8;       // samples per relayout unit: one unit = one round of 16 loads per lane
+constexpr int RL_WARPS = 8;      // relayout warps per CTA
+constexpr int RL_XBYTES = 1024;  // span bytes of one row piece per relayout unit
 
 constexpr int TC_RING = 4;  // depth of the per-CTA ring that passes scheduled tile indices between warp roles
 
@@ -131,9 +145,21 @@ struct TcRing {
     }
 };
 
+// four ci4 bytes (re = high nibble, im = low nibble, two's complement: include/bfxcorr.h) ->
+// eight sign-extended int8: re0 im0 re1 im1 | re2 im2 re3 im3
+__device__ __forceinline__ void tc_widen_ci4(uint32_t w, uint32_t& o0, uint32_t& o1)
+{
+    const uint32_t ure = (w >> 4) & 0x0F0F0F0Fu, uim = w & 0x0F0F0F0Fu;
+    // bit 3 of a nibble set -> OR 0xF0 into its byte (bit3 * 0x1E = bits 4..7)
+    const uint32_t sre = ure | ((ure & 0x08080808u) * 0x1Eu);
+    const uint32_t sim = uim | ((uim & 0x08080808u) * 0x1Eu);
+    o0 = __byte_perm(sre, sim, 0x5140);
+    o1 = __byte_perm(sre, sim, 0x7362);
+}
+
 template <bool CI4>
 __global__ void __launch_bounds__(TcCfg<CI4>::kThreads, 1)
-xcorr_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ CUtensorMap pmap, const TcParams p)
+xcorr_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
 {
     using Cfg = TcCfg<CI4>;
     constexpr int S = Cfg::kOpStages;
@@ -162,7 +188,6 @@ xcorr_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_cons
 
     if (warp == 0 && lane == 0) {
         ptx::prefetch_tensormap(&tmap);
-        ptx::prefetch_tensormap(&pmap);
         for (int s = 0; s < S; ++s) {
             ptx::mbar_init(bar_full + 8 * s, CI4 ? 4 : 1);
             ptx::mbar_init(bar_empty + 8 * s, 1);
@@ -178,7 +203,8 @@ xcorr_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_cons
             }
         for (int s = 0; s < TC_RING; ++s) {
             ptx::mbar_init(bar_sfull + 8 * s, 1);
-            ptx::mbar_init(bar_sempty + 8 * s, CI4 ? 9 : 5);  // MMA issuer + 4 epilogue warps (+ 4 unpack warps)
+            // MMA issuer + 4 epilogue warps (+ 4 unpack warps)
+            ptx::mbar_init(bar_sempty + 8 * s, CI4 ? 9 : 5);
         }
         ptx::fence_barrier_init();
     }
@@ -199,6 +225,7 @@ xcorr_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_cons
         // ===================== TMA producer (S1 for ci8, first half of S1 for ci4) =====================
         if (lane == 0) {
             uint32_t stage = 0, phase = 0;
+            int ready_chan = -1;
             constexpr int NST = CI4 ? R : S;
             for (uint32_t n = 0;; ++n) {
                 ring.wait_free(n);
@@ -209,20 +236,22 @@ xcorr_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_cons
                 const int c = static_cast<int>(w / p.tiles_per_chan);
                 const int q = static_cast<int>(w % p.tiles_per_chan);
                 const TcTile tl = p.tiles[q];
-                // The operand boxes are 64..128-byte pieces of rows that lie nchan*row bytes apart: fetched on
-                // demand they reach DRAM as scattered short bursts and every TMA load waits a DRAM latency.
-                // So the tiles of channel c share out the job of pulling channel c + pf_dist into the L2 as
-                // whole rows, and the operand loads further down become L2 hits.
-                if (c + p.pf_dist < p.nchan) {
-                    const int units = nkb * p.pf_nx;
-                    for (int u = q; u < units; u += p.tiles_per_chan)
-                        ptx::tma_prefetch_l2_3d(&pmap, (u % p.pf_nx) * p.pf_bx, c + p.pf_dist, (u / p.pf_nx) * TC_KT);
+                if (!CI4 && p.rl_enabled && c != ready_chan) {
+                    // the relayout warps (of any CTA) must have
+                    // written all of z[c]; their generic-proxy stores are then ordered before our TMA (async proxy) reads
+                    const unsigned long long want = p.epoch * static_cast<unsigned long long>(p.rl_units);
+                    uint32_t spins = 0;
+                    while (ptx::ld_acquire_u64(p.ready + c) < want)
+                        if (++spins > (1u << 26)) __trap();
+                    ptx::fence_proxy_async_global();
+                    ready_chan = c;
                 }
                 const int xbytes = CI4 ? 64 : 128;  // bytes of one 64-input block in a span row
                 const int xa = tl.row_blk * xbytes;
                 const int xb = tl.col_blk * 2 * xbytes;
                 const uint32_t box = CI4 ? TC_RAW_BOX_BYTES : TC_BOX_BYTES;
                 const uint32_t nbytes = box * (tl.nbox + (tl.a_alias < 0 ? 1 : 0));
+                const int cs = (!CI4 && p.rl_enabled) ? c % p.ring_w : c;  // channel coordinate in the operand source
                 for (int kb = 0; kb < nkb; ++kb) {
                     const uint32_t fullb = (CI4 ? bar_rfull : bar_full) + 8 * stage;
                     const uint32_t emptyb = (CI4 ? bar_rempty : bar_empty) + 8 * stage;
@@ -230,9 +259,9 @@ xcorr_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_cons
                     ptx::mbar_expect_tx(fullb, nbytes);
                     const uint32_t dst = CI4 ? raw_base + stage * TC_RAW_STAGE_BYTES : op_base + stage * TC_STAGE_BYTES;
                     const int t0 = kb * TC_KT;
-                    if (tl.a_alias < 0) ptx::tma_load_3d(dst, &tmap, fullb, xa, c, t0);
-                    ptx::tma_load_3d(dst + box, &tmap, fullb, xb, c, t0);
-                    if (tl.nbox > 1) ptx::tma_load_3d(dst + 2 * box, &tmap, fullb, xb + xbytes, c, t0);
+                    if (tl.a_alias < 0) ptx::tma_load_3d(dst, &tmap, fullb, xa, cs, t0);
+                    ptx::tma_load_3d(dst + box, &tmap, fullb, xb, cs, t0);
+                    if (tl.nbox > 1) ptx::tma_load_3d(dst + 2 * box, &tmap, fullb, xb + xbytes, cs, t0);
                     if (++stage == NST) { stage = 0; phase ^= 1; }
                 }
             }
@@ -267,6 +296,8 @@ xcorr_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_cons
                     if (++stage == S) { stage = 0; phase ^= 1; }
                 }
                 ptx::mma_commit(bar_tfull + 8 * buf);
+                // every operand load of this tile has landed in shared memory: its ring slab may be recycled
+                if (!CI4 && p.rl_enabled) ptx::red_release_add_u64(p.done + w / p.tiles_per_chan, 1ull);
             }
         }
     } else if (warp >= 4 && warp < 8) {
@@ -425,6 +456,83 @@ xcorr_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_cons
         }
     }
 
+    else if (!CI4 && warp >= 8 && p.rl_enabled) {
+        // ===================== relayout warps (S1: unpack-and-transpose, span -> ring z) =====================
+        // A unit = RL_ROWS samples x one 1 KiB piece of the (t, c) row of channel cc: read with coalesced 16-byte
+        // loads (each span byte exactly once per launch), ci4 widened to sign-extended int8 pairs, written with
+        // 16-byte stores to the channel's slab.  Each warp works on its own units.
+        const long long src_pitch = static_cast<long long>(p.nchan) * p.row_in;
+        const int row_out = 2 * p.ninputs;
+        auto do_unit = [&](int cc, int u) {
+            if (cc >= p.ring_w) {
+                // the slab is still owned by channel cc - ring_w until all of its tiles have loaded their operands
+                if (lane == 0) {
+                    const unsigned long long want = p.epoch * static_cast<unsigned long long>(p.tiles_per_chan);
+                    uint32_t spins = 0;
+                    while (ptx::ld_acquire_u64(p.done + (cc - p.ring_w)) < want) {
+                        __nanosleep(256);
+                        if (++spins > (1u << 24)) __trap();
+                    }
+                }
+                __syncwarp();
+            }
+            const int t0 = (u / p.rl_nx) * RL_ROWS;
+            const int xb0 = (u % p.rl_nx) * RL_XBYTES;
+            const int nt = min(RL_ROWS, p.ntime - t0);
+            const int nv = min(RL_XBYTES, p.row_in - xb0) >> 4;  // 16-byte vectors per row piece
+            const int total = nt * nv;
+            const int nv_shift = (nv & (nv - 1)) == 0 ? 31 - __clz(nv) : -1;  // rows are usually 64 vectors: avoid the division
+            const uint8_t* src = p.x + (static_cast<long long>(t0) * p.nchan + cc) * p.row_in + xb0;
+            uint8_t* dst = p.z + (static_cast<long long>(cc % p.ring_w) * p.ntime + t0) * row_out + (p.rl_ci4 ? 2 * xb0 : xb0);
+            constexpr int U = 16;
+            for (int base = static_cast<int>(lane); base < total; base += U * 32) {
+                uint4 v[U];
+#pragma unroll
+                for (int k = 0; k < U; ++k) {
+                    const int idx = base + 32 * k;
+                    const int r = nv_shift >= 0 ? idx >> nv_shift : idx / nv;
+                    if (idx < total) v[k] = ptx::ld_global_stream_v4(src + r * src_pitch + (idx - r * nv) * 16);
+                }
+#pragma unroll
+                for (int k = 0; k < U; ++k) {
+                    const int idx = base + 32 * k;
+                    const int r = nv_shift >= 0 ? idx >> nv_shift : idx / nv;
+                    const int vi = idx - r * nv;
+                    if (idx < total) {
+                        if (p.rl_ci4) {
+                            uint8_t* d = dst + static_cast<long long>(r) * row_out + vi * 32;
+                            uint4 a, b;
+                            tc_widen_ci4(v[k].x, a.x, a.y);
+                            tc_widen_ci4(v[k].y, a.z, a.w);
+                            tc_widen_ci4(v[k].z, b.x, b.y);
+                            tc_widen_ci4(v[k].w, b.z, b.w);
+                            ptx::st_global_v4(d, a);
+                            ptx::st_global_v4(d + 16, b);
+                        } else {
+                            ptx::st_global_v4(dst + static_cast<long long>(r) * row_out + vi * 16, v[k]);
+                        }
+                    }
+                }
+            }
+            // publish: this warp's stores -> visible device-wide and to the TMA (async proxy) readers
+            __threadfence();
+            ptx::fence_proxy_async_global();
+            __syncwarp();
+            if (lane == 0) ptx::red_release_add_u64(p.ready + cc, 1ull);
+        };
+        // Units are handed out channel-major by one global counter, independently of the tile scheduler: the relayout
+        // warps of all CTAs run ahead of the contraction as far as the ring allows (do_unit waits for the slab's
+        // previous channel to be done), so the span's DRAM / address-translation latency is off the critical path.
+        const long long total_units = static_cast<long long>(p.nchan) * p.rl_units;
+        for (;;) {
+            long long u = 0;
+            if (lane == 0) u = static_cast<long long>(atomicAdd(p.sched + 2, 1ull));
+            u = __shfl_sync(0xffffffffu, u, 0);
+            if (u >= total_units) break;
+            do_unit(static_cast<int>(u / p.rl_units), static_cast<int>(u % p.rl_units));
+        }
+    }
+
     ptx::tc_fence_before();
     __syncthreads();
     if (warp == 2) ptx::tmem_dealloc<1>(tmem_base, TC_TMEM_COLS);
@@ -432,6 +540,7 @@ xcorr_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_cons
     if (threadIdx.x == 0 && atomicAdd(p.sched + 1, 1ull) == gridDim.x - 1) {
         p.sched[0] = 0;
         p.sched[1] = 0;
+        p.sched[2] = 0;
     }
 }
 
