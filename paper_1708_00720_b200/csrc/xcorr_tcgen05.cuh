@@ -87,7 +87,16 @@ struct TcParams {
     unsigned long long epoch;  // 1, 2, ... : launch number of this plan
 };
 
-constexpr int RL_ROWS = 8;       // samples per relayout unit: one unit = one round of 16 loads per lane
+#ifndef BFX_RL_ROWS
+#define BFX_RL_ROWS 8
+#endif
+#ifndef BFX_RL_SLEEP
+#define BFX_RL_SLEEP 500
+#endif
+#ifndef BFX_RL_FENCE
+#define BFX_RL_FENCE 0
+#endif
+constexpr int RL_ROWS = BFX_RL_ROWS;      // samples per relayout unit (4 rounds of 16 loads per lane, one release per unit)
 constexpr int RL_WARPS = 8;      // relayout warps per CTA
 constexpr int RL_XBYTES = 1024;  // span bytes of one row piece per relayout unit
 
@@ -470,7 +479,7 @@ xcorr_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
                     const unsigned long long want = p.epoch * static_cast<unsigned long long>(p.tiles_per_chan);
                     uint32_t spins = 0;
                     while (ptx::ld_acquire_u64(p.done + (cc - p.ring_w)) < want) {
-                        __nanosleep(256);
+                        __nanosleep(BFX_RL_SLEEP);
                         if (++spins > (1u << 24)) __trap();
                     }
                 }
@@ -514,8 +523,9 @@ xcorr_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
                     }
                 }
             }
-            // publish: this warp's stores -> visible device-wide and to the TMA (async proxy) readers
-            __threadfence();
+            // publish: every lane's stores are ordered before lane 0's release by the warp barrier (the release is
+            // cumulative), and made visible to the TMA (async proxy) readers by the proxy fence
+            if (BFX_RL_FENCE) __threadfence();
             ptx::fence_proxy_async_global();
             __syncwarp();
             if (lane == 0) ptx::red_release_add_u64(p.ready + cc, 1ull);
