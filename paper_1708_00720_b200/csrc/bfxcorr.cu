@@ -11,6 +11,7 @@
 
 #include "../../include/bfxcorr.h"
 #include "xcorr_simt.cuh"
+#include "xcorr_pair.cuh"
 #include "xcorr_tcgen05.cuh"
 
 namespace {
@@ -18,6 +19,7 @@ namespace {
 using bfx::TcCfg;
 using bfx::TcParams;
 using bfx::TcTile;
+using bfx::PrTile;
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
@@ -36,7 +38,8 @@ struct bfXcorr_impl {
     int last_cuda_error;
     int last_launch_count;
     // S2: lower-triangle tile table (device copy) for the tcgen05 kernel
-    TcTile* d_tiles;
+    TcTile* d_tiles;      // 1-CTA kernel (ninputs <= 64)
+    PrTile* d_pair_tiles; // CTA-pair kernel (ninputs > 64)
     int tiles_per_chan;
     unsigned long long* d_sched;  // dynamic tile scheduler state, re-armed by the kernel itself
     EncodeTiledFn encode;
@@ -95,6 +98,16 @@ std::vector<TcTile> build_tiles(int ninputs)
             tiles.push_back(t);
         }
     }
+    return tiles;
+}
+
+// S2 for the CTA-pair kernel: 128 x 128-input tiles on or below the diagonal, row-major.
+std::vector<PrTile> build_pair_tiles(int ninputs)
+{
+    std::vector<PrTile> tiles;
+    const int nb = (ninputs + bfx::PR_BLK - 1) / bfx::PR_BLK;
+    for (int r = 0; r < nb; ++r)
+        for (int cb = 0; cb <= r; ++cb) tiles.push_back(PrTile{static_cast<int16_t>(r), static_cast<int16_t>(cb)});
     return tiles;
 }
 
@@ -171,10 +184,32 @@ int launch_tcgen05(bfXcorr p, const void* in, void* out, int accumulate, cudaStr
         prm.done = p->d_flags + p->nchan;
         prm.epoch = ++p->epoch;
     }
-    const long long want = prm.ntiles < p->num_sms ? prm.ntiles : p->num_sms;
-    const dim3 grid(static_cast<unsigned>(want));
-    bfx::xcorr_tcgen05_kernel<CI4><<<grid, TcCfg<CI4>::kThreads, TcCfg<CI4>::kSmemBytes, stream>>>(tmap, prm);
-    const cudaError_t e = cudaGetLastError();
+    cudaError_t e = cudaSuccess;
+    if (fused) {
+        // one cluster of two CTAs per tile in flight
+        prm.pair_tiles = p->d_pair_tiles;
+        long long pairs = p->num_sms / 2;
+        if (prm.ntiles < pairs) pairs = prm.ntiles;
+        cudaLaunchConfig_t cfg;
+        std::memset(&cfg, 0, sizeof(cfg));
+        cfg.gridDim = dim3(static_cast<unsigned>(2 * pairs));
+        cfg.blockDim = dim3(bfx::PR_THREADS);
+        cfg.dynamicSmemBytes = bfx::PR_SMEM_BYTES;
+        cfg.stream = stream;
+        cudaLaunchAttribute attr;
+        attr.id = cudaLaunchAttributeClusterDimension;
+        attr.val.clusterDim.x = 2;
+        attr.val.clusterDim.y = 1;
+        attr.val.clusterDim.z = 1;
+        cfg.attrs = &attr;
+        cfg.numAttrs = 1;
+        e = cudaLaunchKernelEx(&cfg, bfx::xcorr_pair_kernel, tmap, prm);
+    } else {
+        const long long want = prm.ntiles < p->num_sms ? prm.ntiles : p->num_sms;
+        const dim3 grid(static_cast<unsigned>(want));
+        bfx::xcorr_tcgen05_kernel<CI4><<<grid, TcCfg<CI4>::kThreads, TcCfg<CI4>::kSmemBytes, stream>>>(tmap, prm);
+    }
+    if (e == cudaSuccess) e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(p, e);
     p->last_launch_count += 1;
     return BF_XCORR_OK;
@@ -238,20 +273,29 @@ int bfXcorrCreate(bfXcorr* plan, int ninputs, int nchan, int ntime, int dtype)
     }
     p->encode = reinterpret_cast<EncodeTiledFn>(fn);
 
-    const std::vector<TcTile> tiles = build_tiles(ninputs);
-    p->tiles_per_chan = static_cast<int>(tiles.size());
-    e = cudaMalloc(reinterpret_cast<void**>(&p->d_tiles), tiles.size() * sizeof(TcTile));
-    if (e == cudaSuccess) e = cudaMemcpy(p->d_tiles, tiles.data(), tiles.size() * sizeof(TcTile), cudaMemcpyHostToDevice);
+    const bool pair = ninputs > bfx::TC_BM_IN;  // more than one tile per channel: CTA pairs + fused S1
+    if (pair) {
+        const std::vector<PrTile> tiles = build_pair_tiles(ninputs);
+        p->tiles_per_chan = static_cast<int>(tiles.size());
+        e = cudaMalloc(reinterpret_cast<void**>(&p->d_pair_tiles), tiles.size() * sizeof(PrTile));
+        if (e == cudaSuccess)
+            e = cudaMemcpy(p->d_pair_tiles, tiles.data(), tiles.size() * sizeof(PrTile), cudaMemcpyHostToDevice);
+    } else {
+        const std::vector<TcTile> tiles = build_tiles(ninputs);
+        p->tiles_per_chan = static_cast<int>(tiles.size());
+        e = cudaMalloc(reinterpret_cast<void**>(&p->d_tiles), tiles.size() * sizeof(TcTile));
+        if (e == cudaSuccess) e = cudaMemcpy(p->d_tiles, tiles.data(), tiles.size() * sizeof(TcTile), cudaMemcpyHostToDevice);
+    }
     if (e == cudaSuccess) e = cudaMalloc(reinterpret_cast<void**>(&p->d_sched), 4 * sizeof(unsigned long long));
     if (e == cudaSuccess) e = cudaMemset(p->d_sched, 0, 4 * sizeof(unsigned long long));
     // A channel whose tiles re-read its samples is first rewritten channel-major (xcorr_relayout.cuh); with a
     // single tile per channel (ninputs <= 64) every sample is read once anyway and the span is used in place.
-    if (e == cudaSuccess && p->tiles_per_chan > 1) {
+    if (e == cudaSuccess && pair) {
         // window = channels the grid works on at once (doubled: producers run a tile or two ahead of their loads);
         // on top of that the ring holds ~16 MiB of look-ahead, so a slab is complete long before its first tile is
         // drawn and stays L2-resident until its last tile is done
         const unsigned long long slab = static_cast<unsigned long long>(ntime) * ninputs * 2ull;
-        const int window = (p->num_sms + p->tiles_per_chan - 1) / p->tiles_per_chan;
+        const int window = (p->num_sms / 2 + p->tiles_per_chan - 1) / p->tiles_per_chan;
         long long ahead = static_cast<long long>((16ull << 20) / slab);
         if (ahead < 2) ahead = 2;
         long long ring = 2 * window + 2 + ahead;
@@ -262,6 +306,8 @@ int bfXcorrCreate(bfXcorr* plan, int ninputs, int nchan, int ntime, int dtype)
         if (e == cudaSuccess) e = cudaMemset(p->d_flags, 0, 2ull * nchan * sizeof(unsigned long long));
     }
     if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(bfx::xcorr_pair_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bfx::PR_SMEM_BYTES);
+    if (e == cudaSuccess)
         e = cudaFuncSetAttribute(bfx::xcorr_tcgen05_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  TcCfg<false>::kSmemBytes);
     if (e == cudaSuccess)
@@ -270,6 +316,7 @@ int bfXcorrCreate(bfXcorr* plan, int ninputs, int nchan, int ntime, int dtype)
     if (e != cudaSuccess) {
         const int st = cuda_fail(nullptr, e);
         if (p->d_tiles) cudaFree(p->d_tiles);
+        if (p->d_pair_tiles) cudaFree(p->d_pair_tiles);
         if (p->d_sched) cudaFree(p->d_sched);
         if (p->d_z) cudaFree(p->d_z);
         if (p->d_flags) cudaFree(p->d_flags);
@@ -318,6 +365,7 @@ int bfXcorrDestroy(bfXcorr plan)
 {
     if (!valid(plan)) return BF_XCORR_INVALID_HANDLE;
     if (plan->d_tiles) cudaFree(plan->d_tiles);
+    if (plan->d_pair_tiles) cudaFree(plan->d_pair_tiles);
     if (plan->d_sched) cudaFree(plan->d_sched);
     if (plan->d_stage_in) cudaFree(plan->d_stage_in);
     if (plan->d_z) cudaFree(plan->d_z);

@@ -70,6 +70,13 @@ __device__ __forceinline__ void mbar_arrive_cluster(uint32_t bar, uint32_t cta)
         : "memory");
 }
 
+// arrive on a barrier given by its shared::cluster address (mapa result)
+// (default .release.cta semantics: no data is published through these arrivals, only "I am done")
+__device__ __forceinline__ void mbar_arrive_cluster_addr(uint32_t cluster_bar)
+{
+    asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cluster_bar) : "memory");
+}
+
 __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity)
 {
     uint32_t ok;
@@ -260,6 +267,12 @@ __device__ __forceinline__ void tma_prefetch_l2_3d(const CUtensorMap* m, int x, 
                  : "memory");
 }
 
+// pull [p, p + bytes) into the L2 (p 16-byte aligned, bytes a multiple of 16); no completion tracking
+__device__ __forceinline__ void bulk_prefetch_l2(const void* p, uint32_t bytes)
+{
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+}
+
 __device__ __forceinline__ void red_add_global_v2(int32_t* p, int2 v)
 {
     asm volatile("red.global.add.u32 [%0], %1;\n\tred.global.add.u32 [%0+4], %2;" ::"l"(p), "r"(v.x), "r"(v.y) : "memory");
@@ -271,6 +284,12 @@ __device__ __forceinline__ unsigned long long ld_acquire_u64(const unsigned long
     unsigned long long v;
     asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
     return v;
+}
+
+// no release: used where the event being counted was itself observed through an acquire by this thread
+__device__ __forceinline__ void red_relaxed_add_u64(unsigned long long* p, unsigned long long v)
+{
+    asm volatile("red.relaxed.gpu.global.add.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
 }
 
 __device__ __forceinline__ void red_release_add_u64(unsigned long long* p, unsigned long long v)

@@ -34,7 +34,10 @@ namespace bfx {
 // ---- tile geometry ----------------------------------------------------------------------------
 constexpr int TC_BM_IN = 64;    // inputs per A tile  -> UMMA M = 128 real rows
 constexpr int TC_BN_IN = 128;   // inputs per B tile  -> UMMA N = 256 real columns (two 64-input boxes)
-constexpr int TC_KT = 64;       // samples per pipeline stage (2 MMAs of K = 32)
+#ifndef BFX_KT
+#define BFX_KT 128
+#endif
+constexpr int TC_KT = BFX_KT;   // samples per pipeline stage (TC_KT / 32 MMAs of K = 32); one TMA box = TC_KT rows
 constexpr int TC_BOX_BYTES = TC_KT * 128;        // one operand box: KT rows of 128 bytes
 constexpr int TC_STAGE_BYTES = 3 * TC_BOX_BYTES; // A, B0, B1
 constexpr int TC_RAW_BOX_BYTES = TC_KT * 64;     // ci4: one raw box, KT rows of 64 bytes
@@ -48,8 +51,8 @@ constexpr int TC_TMEM_COLS = 512;                // two 256-column accumulators
 
 template <bool CI4>
 struct TcCfg {
-    static constexpr int kOpStages = CI4 ? 4 : 6;   // int8 operand ring the MMA reads
-    static constexpr int kRawStages = CI4 ? 4 : 0;  // ci4: raw byte ring the TMA fills
+    static constexpr int kOpStages = (CI4 ? 4 : 6) * 64 / TC_KT;   // int8 operand ring the MMA reads
+    static constexpr int kRawStages = CI4 ? 4 * 64 / TC_KT : 0;  // ci4: raw byte ring the TMA fills
     static constexpr int kThreads = CI4 ? 384 : 512;  // direct ci4: 4 unpack warps; else up to 8 relayout warps
     static constexpr int kSmemBytes = 1024 /*align slack*/ + kOpStages * TC_STAGE_BYTES +
                                       kRawStages * TC_RAW_STAGE_BYTES + TC_STG_BYTES + 512 /*barriers*/;
@@ -66,7 +69,8 @@ struct TcTile {
 
 struct TcParams {
     int32_t* out;
-    const TcTile* tiles;
+    const TcTile* tiles;     // 1-CTA kernel: 64 x 128-input tiles
+    const void* pair_tiles;  // CTA-pair kernel: 128 x 128-input tiles (PrTile)
     int ninputs, nchan, ntime;
     int tiles_per_chan;
     long long ntiles;  // tiles_per_chan * nchan
@@ -164,6 +168,181 @@ __device__ __forceinline__ void tc_widen_ci4(uint32_t w, uint32_t& o0, uint32_t&
     const uint32_t sim = uim | ((uim & 0x08080808u) * 0x1Eu);
     o0 = __byte_perm(sre, sim, 0x5140);
     o1 = __byte_perm(sre, sim, 0x7362);
+}
+
+// ===================== one epilogue chunk (S4): 32 TMEM lanes x 128 columns -> 16 rows x 64 visibilities ==========
+// TMEM lane = real row m = 2 i + part of the A block, so lanes (2k, 2k+1) hold the re and im rows of input row
+// i0 + k.  One shuffle per column pair forms Re V (even lane) / Im V (odd lane); both lanes store their 4-byte
+// half of the visibility into a per-warp staging row (conflict free: pitch = 130 words).  Lanes 0..15 then each
+// own one packed-triangle row segment of <= 64 visibilities and hand it to the TMA unit: a bulk store
+// (accumulate = 0) or a bulk int32 reduce-add performed at the L2 (accumulate != 0), so the old values never
+// travel to the SM.  Bulk copies need 16-byte alignment but triangle rows are only 8-byte aligned: a staging row
+// is placed in a slot of the same address parity as its global start (rows i = 1, 2 mod 4 start on an odd
+// visibility; i0 is a multiple of 16, jb of 64) and an odd head / tail visibility goes out as a scalar store / red.
+// release_bar != 0: local shared address of the "accumulator drained" barrier to arrive on (cluster address of
+// the leader CTA's barrier in the pair kernel) once this warp's TMEM reads are done.
+template <bool SHIFT8, bool REMOTE_RELEASE = false>
+__device__ __forceinline__ void tc_epilogue_chunk(const TcParams& p, uint32_t lane, uint32_t tcol, uint32_t stg_buf,
+                                                  int32_t* out_c, int i0, int jb, uint32_t release_bar)
+{
+    const uint32_t par = lane & 1;                // 0: re row of its input, 1: im row
+    const int sgn = par ? -1 : 1;
+    const uint32_t krow = lane >> 1;
+    const uint32_t wr_off = (krow ^ ((krow >> 1) & 1)) * TC_STG_PITCH + 4 * par;
+    const uint32_t own_off = (lane ^ ((lane >> 1) & 1)) * TC_STG_PITCH;  // lanes 0..15: slot of row `lane`
+    // the bulk group that read this staging buffer two chunks ago must be done with it
+    if (lane < 16) ptx::bulk_wait_read<1>();
+    __syncwarp();
+#ifdef BFX_PROBE_NO_EPI
+    if (release_bar) {
+        ptx::tc_fence_before();
+        __syncwarp();
+        if (lane == 0) {
+            if (REMOTE_RELEASE) ptx::mbar_arrive_cluster_addr(release_bar); else ptx::mbar_arrive(release_bar);
+        }
+    }
+    return;
+#endif
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        uint32_t g[32];
+        ptx::tmem_ld_32x32b_x32(tcol + q * 32, g);
+        ptx::tmem_ld_wait();
+#pragma unroll
+        for (int k = 0; k < 16; ++k) {
+            int ge = static_cast<int>(g[2 * k]), go = static_cast<int>(g[2 * k + 1]);
+            if (SHIFT8) { ge >>= 8; go >>= 8; }       // G came out scaled by 16*16, exactly
+            const int v = __shfl_xor_sync(0xffffffffu, go, 1);
+            // even lane: Re V[i][j] = G[2i][2j] + G[2i+1][2j+1]; odd lane: Im V[i][j] = G[2i+1][2j] - G[2i][2j+1]
+            const int val = ge + sgn * v;
+            asm volatile("st.shared.s32 [%0], %1;" ::"r"(stg_buf + wr_off + (q * 16 + k) * 8), "r"(val) : "memory");
+        }
+    }
+    if (release_bar) {
+        // all TMEM reads of this accumulator are done: hand it back to the MMA issuer
+        ptx::tc_fence_before();
+        __syncwarp();
+        if (lane == 0) {
+            if (REMOTE_RELEASE) ptx::mbar_arrive_cluster_addr(release_bar); else ptx::mbar_arrive(release_bar);
+        }
+    }
+    ptx::fence_proxy_async_smem();  // staging writes -> visible to the bulk-copy engine
+    __syncwarp();
+#ifdef BFX_PROBE_NO_STORE
+    return;
+#endif
+    if (lane < 16) {
+        const int i_own = i0 + static_cast<int>(lane);
+        int n = i_own + 1 - jb;       // row i holds columns j <= i only (S2 masking of diagonal tiles)
+        n = n > TC_CJ ? TC_CJ : n;
+        if (i_own >= p.ninputs) n = 0;
+        if (n > 0) {
+            const long long e0 = static_cast<long long>(i_own) * (i_own + 1) / 2 + jb;
+            int32_t* const g0 = out_c + 2 * e0;
+            const uint32_t s0 = stg_buf + own_off;
+            const int head = static_cast<int>(e0 & 1);
+            const int nbulk = (n - head) & ~1;
+            if (head) {
+                int2 v;
+                asm volatile("ld.shared.v2.s32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(s0));
+                if (p.accumulate) ptx::red_add_global_v2(g0, v); else ptx::st_global_v2(g0, v);
+            }
+            if (nbulk > 0) {
+                if (p.accumulate) ptx::bulk_reduce_add_s32(g0 + 2 * head, s0 + 8 * head, 8u * nbulk);
+                else ptx::bulk_store(g0 + 2 * head, s0 + 8 * head, 8u * nbulk);
+            }
+            if (head + nbulk < n) {
+                int2 v;
+                asm volatile("ld.shared.v2.s32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(s0 + 8 * (n - 1)));
+                if (p.accumulate) ptx::red_add_global_v2(g0 + 2 * (n - 1), v); else ptx::st_global_v2(g0 + 2 * (n - 1), v);
+            }
+        }
+        ptx::bulk_commit();
+    }
+}
+
+// ===================== relayout warps (S1: unpack-and-transpose, span -> ring z) =====================
+// Shared by the 1-CTA and the CTA-pair kernels; run by whole warps.
+__device__ __forceinline__ void tc_relayout_role(const TcParams& p, uint32_t lane)
+{
+#ifdef BFX_PROBE_NO_RL
+    return;
+#endif
+    // ===================== relayout warps (S1: unpack-and-transpose, span -> ring z) =====================
+    // A unit = RL_ROWS samples x one 1 KiB piece of the (t, c) row of channel cc: read with coalesced 16-byte
+    // loads (each span byte exactly once per launch), ci4 widened to sign-extended int8 pairs, written with
+    // 16-byte stores to the channel's slab.  Each warp works on its own units.
+    const long long src_pitch = static_cast<long long>(p.nchan) * p.row_in;
+    const int row_out = 2 * p.ninputs;
+    auto do_unit = [&](int cc, int u) {
+        if (cc >= p.ring_w) {
+            // the slab is still owned by channel cc - ring_w until all of its tiles have loaded their operands
+            if (lane == 0) {
+                const unsigned long long want = p.epoch * static_cast<unsigned long long>(p.tiles_per_chan);
+                uint32_t spins = 0;
+                while (ptx::ld_acquire_u64(p.done + (cc - p.ring_w)) < want) {
+                    __nanosleep(BFX_RL_SLEEP);
+                    if (++spins > (1u << 24)) __trap();
+                }
+            }
+            __syncwarp();
+        }
+        const int t0 = (u / p.rl_nx) * RL_ROWS;
+        const int xb0 = (u % p.rl_nx) * RL_XBYTES;
+        const int nt = min(RL_ROWS, p.ntime - t0);
+        const int nv = min(RL_XBYTES, p.row_in - xb0) >> 4;  // 16-byte vectors per row piece
+        const int total = nt * nv;
+        const int nv_shift = (nv & (nv - 1)) == 0 ? 31 - __clz(nv) : -1;  // rows are usually 64 vectors: avoid the division
+        const uint8_t* src = p.x + (static_cast<long long>(t0) * p.nchan + cc) * p.row_in + xb0;
+        uint8_t* dst = p.z + (static_cast<long long>(cc % p.ring_w) * p.ntime + t0) * row_out + (p.rl_ci4 ? 2 * xb0 : xb0);
+        constexpr int U = 16;
+        for (int base = static_cast<int>(lane); base < total; base += U * 32) {
+            uint4 v[U];
+#pragma unroll
+            for (int k = 0; k < U; ++k) {
+                const int idx = base + 32 * k;
+                const int r = nv_shift >= 0 ? idx >> nv_shift : idx / nv;
+                if (idx < total) v[k] = ptx::ld_global_stream_v4(src + r * src_pitch + (idx - r * nv) * 16);
+            }
+#pragma unroll
+            for (int k = 0; k < U; ++k) {
+                const int idx = base + 32 * k;
+                const int r = nv_shift >= 0 ? idx >> nv_shift : idx / nv;
+                const int vi = idx - r * nv;
+                if (idx < total) {
+                    if (p.rl_ci4) {
+                        uint8_t* d = dst + static_cast<long long>(r) * row_out + vi * 32;
+                        uint4 a, b;
+                        tc_widen_ci4(v[k].x, a.x, a.y);
+                        tc_widen_ci4(v[k].y, a.z, a.w);
+                        tc_widen_ci4(v[k].z, b.x, b.y);
+                        tc_widen_ci4(v[k].w, b.z, b.w);
+                        ptx::st_global_v4(d, a);
+                        ptx::st_global_v4(d + 16, b);
+                    } else {
+                        ptx::st_global_v4(dst + static_cast<long long>(r) * row_out + vi * 16, v[k]);
+                    }
+                }
+            }
+        }
+        // publish: every lane's stores are ordered before lane 0's release by the warp barrier (the release is
+        // cumulative), and made visible to the TMA (async proxy) readers by the proxy fence
+        if (BFX_RL_FENCE) __threadfence();
+        ptx::fence_proxy_async_global();
+        __syncwarp();
+        if (lane == 0) ptx::red_release_add_u64(p.ready + cc, 1ull);
+    };
+    // Units are handed out channel-major by one global counter, independently of the tile scheduler: the relayout
+    // warps of all CTAs run ahead of the contraction as far as the ring allows (do_unit waits for the slab's
+    // previous channel to be done), so the span's DRAM / address-translation latency is off the critical path.
+    const long long total_units = static_cast<long long>(p.nchan) * p.rl_units;
+    for (;;) {
+        long long u = 0;
+        if (lane == 0) u = static_cast<long long>(atomicAdd(p.sched + 2, 1ull));
+        u = __shfl_sync(0xffffffffu, u, 0);
+        if (u >= total_units) break;
+        do_unit(static_cast<int>(u / p.rl_units), static_cast<int>(u % p.rl_units));
+    }
 }
 
 template <bool CI4>
@@ -305,28 +484,15 @@ xcorr_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
                     if (++stage == S) { stage = 0; phase ^= 1; }
                 }
                 ptx::mma_commit(bar_tfull + 8 * buf);
-                // every operand load of this tile has landed in shared memory: its ring slab may be recycled
-                if (!CI4 && p.rl_enabled) ptx::red_release_add_u64(p.done + w / p.tiles_per_chan, 1ull);
+                // every operand load of this tile has landed in shared memory (observed through the full barriers, so a
+                // relaxed count is enough): its ring slab may be recycled
+                if (!CI4 && p.rl_enabled) ptx::red_relaxed_add_u64(p.done + w / p.tiles_per_chan, 1ull);
             }
         }
     } else if (warp >= 4 && warp < 8) {
         // ===================== epilogue (S4) =====================
-        // TMEM lane = real row m = 2 i + part of the A block, so lanes (2k, 2k+1) hold the re and im rows of
-        // input row k of this warp.  One shuffle per column pair forms Re V (even lane) / Im V (odd lane);
-        // both lanes store their 4-byte half of the visibility into a per-warp staging row (conflict free:
-        // pitch = 130 words).  Lanes 0..15 then each own one packed-triangle row segment of <= 64
-        // visibilities and hand it to the TMA unit: a bulk store (accumulate = 0) or a bulk int32
-        // reduce-add performed at the L2 (accumulate != 0), so the old values never travel to the SM.
-        // Bulk copies need 16-byte alignment but triangle rows are only 8-byte aligned: a staging row is
-        // placed in a slot of the same address parity as its global start (rows i = 1, 2 mod 4 start on
-        // an odd visibility) and an odd head / tail visibility goes out as a scalar store / red.
         const int wq = warp - 4;                      // TMEM lane quarter
-        const uint32_t par = lane & 1;                // 0: re row of its input, 1: im row
-        const int sgn = par ? -1 : 1;
-        const uint32_t krow = lane >> 1;
         const uint32_t stg_warp = stg_base + wq * TC_STG_WARP_BYTES;
-        const uint32_t wr_off = (krow ^ ((krow >> 1) & 1)) * TC_STG_PITCH + 4 * par;
-        const uint32_t own_off = (lane ^ ((lane >> 1) & 1)) * TC_STG_PITCH;  // lanes 0..15: slot of row `lane`
         const long long nbl = static_cast<long long>(p.ninputs) * (p.ninputs + 1) / 2;
         uint32_t nchunks_done = 0;
         for (uint32_t it = 0;; ++it) {
@@ -339,68 +505,14 @@ xcorr_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
             const int j0 = tl.col_blk * TC_BN_IN;
             const int nchunk = tl.nbox;                       // 64 visibilities columns per chunk
             int32_t* const out_c = p.out + 2 * (static_cast<long long>(c) * nbl);
-            const int i_own = i0 + static_cast<int>(lane);    // lanes 0..15
-            const long long rowk_own = static_cast<long long>(i_own) * (i_own + 1) / 2;
 
             ptx::mbar_wait(bar_tfull + 8 * buf, bphase);
             ptx::tc_fence_after();
             for (int jc = 0; jc < nchunk; ++jc, ++nchunks_done) {
                 const uint32_t stg_buf = stg_warp + (nchunks_done & 1) * TC_STG_BUF_BYTES;
-                // the bulk group that read this staging buffer two chunks ago must be done with it
-                if (lane < 16) ptx::bulk_wait_read<1>();
-                __syncwarp();
                 const uint32_t tcol = tmem_base + (static_cast<uint32_t>(32 * wq) << 16) + buf * 256 + jc * 128;
-#pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    uint32_t g[32];
-                    ptx::tmem_ld_32x32b_x32(tcol + q * 32, g);
-                    ptx::tmem_ld_wait();
-#pragma unroll
-                    for (int k = 0; k < 16; ++k) {
-                        int ge = static_cast<int>(g[2 * k]), go = static_cast<int>(g[2 * k + 1]);
-                        if (CI4) { ge >>= 8; go >>= 8; }       // G came out scaled by 16*16, exactly
-                        const int v = __shfl_xor_sync(0xffffffffu, go, 1);
-                        // even lane: Re V[i][j] = G[2i][2j] + G[2i+1][2j+1]; odd lane: Im V[i][j] = G[2i+1][2j] - G[2i][2j+1]
-                        const int val = ge + sgn * v;
-                        asm volatile("st.shared.s32 [%0], %1;" ::"r"(stg_buf + wr_off + (q * 16 + k) * 8), "r"(val) : "memory");
-                    }
-                }
-                if (jc == nchunk - 1) {
-                    // all TMEM reads of this accumulator are done: hand it back to the MMA issuer
-                    ptx::tc_fence_before();
-                    __syncwarp();
-                    if (lane == 0) ptx::mbar_arrive(bar_tempty + 8 * buf);
-                }
-                ptx::fence_proxy_async_smem();  // staging writes -> visible to the bulk-copy engine
-                __syncwarp();
-                if (lane < 16) {
-                    const int jb = j0 + jc * TC_CJ;
-                    int n = i_own + 1 - jb;       // row i holds columns j <= i only (S2 masking of diagonal tiles)
-                    n = n > TC_CJ ? TC_CJ : n;
-                    if (i_own >= p.ninputs) n = 0;
-                    if (n > 0) {
-                        const long long e0 = rowk_own + jb;
-                        int32_t* const g0 = out_c + 2 * e0;
-                        const uint32_t s0 = stg_buf + own_off;
-                        const int head = static_cast<int>(e0 & 1);
-                        const int nbulk = (n - head) & ~1;
-                        if (head) {
-                            int2 v;
-                            asm volatile("ld.shared.v2.s32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(s0));
-                            if (p.accumulate) ptx::red_add_global_v2(g0, v); else ptx::st_global_v2(g0, v);
-                        }
-                        if (nbulk > 0) {
-                            if (p.accumulate) ptx::bulk_reduce_add_s32(g0 + 2 * head, s0 + 8 * head, 8u * nbulk);
-                            else ptx::bulk_store(g0 + 2 * head, s0 + 8 * head, 8u * nbulk);
-                        }
-                        if (head + nbulk < n) {
-                            int2 v;
-                            asm volatile("ld.shared.v2.s32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(s0 + 8 * (n - 1)));
-                            if (p.accumulate) ptx::red_add_global_v2(g0 + 2 * (n - 1), v); else ptx::st_global_v2(g0 + 2 * (n - 1), v);
-                        }
-                    }
-                    ptx::bulk_commit();
-                }
+                tc_epilogue_chunk<CI4>(p, lane, tcol, stg_buf, out_c, i0, j0 + jc * TC_CJ,
+                                       jc == nchunk - 1 ? bar_tempty + 8 * buf : 0u);
             }
         }
         if (lane < 16) ptx::bulk_wait_read<0>();  // shared memory must outlive the bulk reads
@@ -466,81 +578,7 @@ xcorr_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
     }
 
     else if (!CI4 && warp >= 8 && p.rl_enabled) {
-        // ===================== relayout warps (S1: unpack-and-transpose, span -> ring z) =====================
-        // A unit = RL_ROWS samples x one 1 KiB piece of the (t, c) row of channel cc: read with coalesced 16-byte
-        // loads (each span byte exactly once per launch), ci4 widened to sign-extended int8 pairs, written with
-        // 16-byte stores to the channel's slab.  Each warp works on its own units.
-        const long long src_pitch = static_cast<long long>(p.nchan) * p.row_in;
-        const int row_out = 2 * p.ninputs;
-        auto do_unit = [&](int cc, int u) {
-            if (cc >= p.ring_w) {
-                // the slab is still owned by channel cc - ring_w until all of its tiles have loaded their operands
-                if (lane == 0) {
-                    const unsigned long long want = p.epoch * static_cast<unsigned long long>(p.tiles_per_chan);
-                    uint32_t spins = 0;
-                    while (ptx::ld_acquire_u64(p.done + (cc - p.ring_w)) < want) {
-                        __nanosleep(BFX_RL_SLEEP);
-                        if (++spins > (1u << 24)) __trap();
-                    }
-                }
-                __syncwarp();
-            }
-            const int t0 = (u / p.rl_nx) * RL_ROWS;
-            const int xb0 = (u % p.rl_nx) * RL_XBYTES;
-            const int nt = min(RL_ROWS, p.ntime - t0);
-            const int nv = min(RL_XBYTES, p.row_in - xb0) >> 4;  // 16-byte vectors per row piece
-            const int total = nt * nv;
-            const int nv_shift = (nv & (nv - 1)) == 0 ? 31 - __clz(nv) : -1;  // rows are usually 64 vectors: avoid the division
-            const uint8_t* src = p.x + (static_cast<long long>(t0) * p.nchan + cc) * p.row_in + xb0;
-            uint8_t* dst = p.z + (static_cast<long long>(cc % p.ring_w) * p.ntime + t0) * row_out + (p.rl_ci4 ? 2 * xb0 : xb0);
-            constexpr int U = 16;
-            for (int base = static_cast<int>(lane); base < total; base += U * 32) {
-                uint4 v[U];
-#pragma unroll
-                for (int k = 0; k < U; ++k) {
-                    const int idx = base + 32 * k;
-                    const int r = nv_shift >= 0 ? idx >> nv_shift : idx / nv;
-                    if (idx < total) v[k] = ptx::ld_global_stream_v4(src + r * src_pitch + (idx - r * nv) * 16);
-                }
-#pragma unroll
-                for (int k = 0; k < U; ++k) {
-                    const int idx = base + 32 * k;
-                    const int r = nv_shift >= 0 ? idx >> nv_shift : idx / nv;
-                    const int vi = idx - r * nv;
-                    if (idx < total) {
-                        if (p.rl_ci4) {
-                            uint8_t* d = dst + static_cast<long long>(r) * row_out + vi * 32;
-                            uint4 a, b;
-                            tc_widen_ci4(v[k].x, a.x, a.y);
-                            tc_widen_ci4(v[k].y, a.z, a.w);
-                            tc_widen_ci4(v[k].z, b.x, b.y);
-                            tc_widen_ci4(v[k].w, b.z, b.w);
-                            ptx::st_global_v4(d, a);
-                            ptx::st_global_v4(d + 16, b);
-                        } else {
-                            ptx::st_global_v4(dst + static_cast<long long>(r) * row_out + vi * 16, v[k]);
-                        }
-                    }
-                }
-            }
-            // publish: every lane's stores are ordered before lane 0's release by the warp barrier (the release is
-            // cumulative), and made visible to the TMA (async proxy) readers by the proxy fence
-            if (BFX_RL_FENCE) __threadfence();
-            ptx::fence_proxy_async_global();
-            __syncwarp();
-            if (lane == 0) ptx::red_release_add_u64(p.ready + cc, 1ull);
-        };
-        // Units are handed out channel-major by one global counter, independently of the tile scheduler: the relayout
-        // warps of all CTAs run ahead of the contraction as far as the ring allows (do_unit waits for the slab's
-        // previous channel to be done), so the span's DRAM / address-translation latency is off the critical path.
-        const long long total_units = static_cast<long long>(p.nchan) * p.rl_units;
-        for (;;) {
-            long long u = 0;
-            if (lane == 0) u = static_cast<long long>(atomicAdd(p.sched + 2, 1ull));
-            u = __shfl_sync(0xffffffffu, u, 0);
-            if (u >= total_units) break;
-            do_unit(static_cast<int>(u / p.rl_units), static_cast<int>(u % p.rl_units));
-        }
+        tc_relayout_role(p, lane);
     }
 
     ptx::tc_fence_before();
