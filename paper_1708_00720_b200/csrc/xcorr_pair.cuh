@@ -32,6 +32,21 @@ struct PrTile {
     int16_t col_blk;  // Cb: columns [128 Cb, 128 Cb + 128), Cb <= R
 };
 
+// S2 decode without touching memory: tile index w -> (channel c, row block R, column block Cb <= R), tiles of a
+// channel enumerated row-major over the lower triangle of 128-input blocks: q = R (R + 1) / 2 + Cb.
+struct PrWhere {
+    int c, R, Cb;
+};
+__device__ __forceinline__ PrWhere pr_decode(long long w, int tiles_per_chan)
+{
+    const uint32_t wu = static_cast<uint32_t>(w), tpc = static_cast<uint32_t>(tiles_per_chan);  // ntiles < 2^32 (host-checked)
+    const uint32_t c = wu / tpc, q = wu - c * tpc;
+    int R = static_cast<int>((sqrtf(8.0f * static_cast<float>(q) + 1.0f) - 1.0f) * 0.5f);
+    while (R * (R + 1) / 2 > static_cast<int>(q)) --R;
+    while ((R + 1) * (R + 2) / 2 <= static_cast<int>(q)) ++R;
+    return PrWhere{static_cast<int>(c), R, static_cast<int>(q) - R * (R + 1) / 2};
+}
+
 // wait with cluster-scope acquire: the data guarded by the barrier was written by the peer CTA
 __device__ __forceinline__ void pr_mbar_wait_cluster(uint32_t bar, uint32_t parity)
 {
@@ -121,52 +136,69 @@ xcorr_pair_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
 
     const int nkb = (p.ntime + TC_KT - 1) / TC_KT;
-    const PrTile* const tiles = static_cast<const PrTile*>(p.pair_tiles);
     const PrRing ring{bar_sfull, ring_base, ptx::mapa(bar_sempty, 0)};
     const uint32_t lead_full = ptx::mapa(bar_full, 0);
     const uint32_t lead_tempty = ptx::mapa(bar_tempty, 0);
 
+    // The producer and MMA-issuer loops are run by whole, converged warps with only the asynchronous instructions
+    // predicated on lane 0: all addresses, descriptors and coordinates are then warp-uniform, so the compiler keeps
+    // them in uniform registers and a UTMALDG / UTCIMMA issue costs a few cycles instead of ~80 (measured:
+    // four MMAs per stage issued from a lone thread ran the tensor pipe at 69 %, from a converged warp at 100 %).
     if (warp == 0) {
         // ===================== TMA producer (+ tile scheduler in the leader) =====================
-        if (lane == 0) {
-            uint32_t stage = 0, phase = 0;
-            int ready_chan = -1;
-            for (uint32_t n = 0;; ++n) {
-                long long w;
-                if (leader) {
-                    const uint32_t slot = n % TC_RING;
-                    ptx::mbar_wait(bar_sempty + 8 * slot, ((n / TC_RING) & 1) ^ 1);
-                    w = static_cast<long long>(atomicAdd(p.sched, 1ull));
-                    if (w >= p.ntiles) w = -1;
+        uint32_t stage = 0, phase = 0;
+        int ready_chan = -1;
+        // the leader draws tile n + 1 from the global counter before it loads tile n: the atomic's round trip
+        // (and everything the other roles do on receiving an index) overlaps the loads of the current tile
+        unsigned long long w_next = 0;
+        if (leader) {
+            if (lane == 0) w_next = atomicAdd(p.sched, 1ull);
+            w_next = __shfl_sync(0xffffffffu, w_next, 0);
+        }
+        for (uint32_t n = 0;; ++n) {
+            long long w;
+            if (leader) {
+                const uint32_t slot = n % TC_RING;
+                ptx::mbar_wait(bar_sempty + 8 * slot, ((n / TC_RING) & 1) ^ 1);
+                w = static_cast<long long>(w_next);
+                if (w >= p.ntiles) w = -1;
+                if (lane == 0) {
+                    if (w >= 0) w_next = atomicAdd(p.sched, 1ull);
                     asm volatile("st.shared.s64 [%0], %1;" ::"r"(ring_base + 8 * slot), "l"(w) : "memory");
                     ptx::mbar_arrive(bar_sfull + 8 * slot);
                     asm volatile("st.shared::cluster.s64 [%0], %1;" ::"r"(ptx::mapa(ring_base + 8 * slot, 1)), "l"(w) : "memory");
                     ptx::mbar_arrive_cluster(bar_sfull + 8 * slot, 1);
-                } else {
-                    w = ring.get<false>(n, 0);
                 }
-                if (w < 0) break;
-                const int c = static_cast<int>(w / p.tiles_per_chan);
-                const PrTile tl = tiles[w % p.tiles_per_chan];
-                if (c != ready_chan) {
-                    // the relayout warps (of any CTA) must have written all of z[c]; their generic-proxy stores are
-                    // then ordered before our TMA (async proxy) reads
+                w_next = __shfl_sync(0xffffffffu, w_next, 0);
+            } else {
+                w = __shfl_sync(0xffffffffu, ring.get<true>(n, lane), 0);
+            }
+            if (w < 0) break;
+            const PrWhere tl = pr_decode(w, p.tiles_per_chan);
+            const int c = tl.c;
+            if (c != ready_chan) {
+                // the relayout warps (of any CTA) must have written all of z[c]; their generic-proxy stores are
+                // then ordered before our TMA (async proxy) reads
+                if (lane == 0) {
+#ifndef BFX_PROBE_NO_RL
                     const unsigned long long want = p.epoch * static_cast<unsigned long long>(p.rl_units);
                     uint32_t spins = 0;
-#ifndef BFX_PROBE_NO_RL
                     while (ptx::ld_acquire_u64(p.ready + c) < want)
                         if (++spins > (1u << 26)) __trap();
 #endif
                     ptx::fence_proxy_async_global();
-                    ready_chan = c;
                 }
-                const int cs = c % p.ring_w;
-                const bool diag = tl.row_blk == tl.col_blk;
-                const int xa = 256 * tl.row_blk + 128 * static_cast<int>(rank);
-                const int xb = 256 * tl.col_blk + 128 * static_cast<int>(rank);
-                const uint32_t cta_bytes = diag ? TC_BOX_BYTES : 2 * TC_BOX_BYTES;
-                for (int kb = 0; kb < nkb; ++kb) {
-                    ptx::mbar_wait(bar_empty + 8 * stage, phase ^ 1);
+                __syncwarp();
+                ready_chan = c;
+            }
+            const int cs = c % p.ring_w;
+            const bool diag = tl.R == tl.Cb;
+            const int xa = 256 * tl.R + 128 * static_cast<int>(rank);
+            const int xb = 256 * tl.Cb + 128 * static_cast<int>(rank);
+            const uint32_t cta_bytes = diag ? TC_BOX_BYTES : 2 * TC_BOX_BYTES;
+            for (int kb = 0; kb < nkb; ++kb) {
+                ptx::mbar_wait(bar_empty + 8 * stage, phase ^ 1);
+                if (lane == 0) {
 #ifdef BFX_PROBE_NO_TMA
                     if (leader) ptx::mbar_arrive(bar_full + 8 * stage);
 #else
@@ -177,45 +209,50 @@ xcorr_pair_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
                     ptx::tma_load_3d_cg2(dst, &tmap, fullb, xa, cs, t0);
                     if (!diag) ptx::tma_load_3d_cg2(dst + TC_BOX_BYTES, &tmap, fullb, xb, cs, t0);
 #endif
-                    if (++stage == S) { stage = 0; phase ^= 1; }
                 }
+                __syncwarp();
+                if (++stage == S) { stage = 0; phase ^= 1; }
             }
         }
     } else if (warp == 1) {
         // ===================== MMA issuer (S3), leader only =====================
-        if (leader && lane == 0) {
+        if (leader) {
             uint32_t stage = 0, phase = 0;
             const uint32_t idesc = tc_instr_desc(256, 256);
             for (uint32_t it = 0;; ++it) {
-                const long long w = ring.get<false>(it, 0);
+                const long long w = __shfl_sync(0xffffffffu, ring.get<true>(it, lane), 0);
                 if (w < 0) break;
-                const PrTile tl = tiles[w % p.tiles_per_chan];
-                const bool diag = tl.row_blk == tl.col_blk;
+                const PrWhere tl = pr_decode(w, p.tiles_per_chan);
+                const bool diag = tl.R == tl.Cb;
                 const uint32_t buf = it & 1, bphase = (it >> 1) & 1;
                 const uint32_t d_tmem = tmem_base + buf * 256;
-                pr_mbar_wait_cluster(bar_tempty + 8 * buf, bphase ^ 1);
+                ptx::mbar_wait(bar_tempty + 8 * buf, bphase ^ 1);
                 ptx::tc_fence_after();
                 for (int kb = 0; kb < nkb; ++kb) {
-                    pr_mbar_wait_cluster(bar_full + 8 * stage, phase);
+                    ptx::mbar_wait(bar_full + 8 * stage, phase);
                     ptx::tc_fence_after();
                     const uint32_t sbase = op_base + stage * PR_STAGE_BYTES;
                     const uint64_t adesc = tc_smem_desc(sbase, TC_BOX_BYTES);
                     const uint64_t bdesc = tc_smem_desc(diag ? sbase : sbase + TC_BOX_BYTES, TC_BOX_BYTES);
                     const int trem = p.ntime - kb * TC_KT;
                     const int nk = trem >= TC_KT ? TC_KT / 32 : (trem + 31) / 32;
+                    if (lane == 0) {
 #ifndef BFX_PROBE_NO_MMA
-                    for (int k = 0; k < nk; ++k)
-#else
-                    for (int k = 0; k < 0; ++k)
+                        for (int k = 0; k < nk; ++k)
+                            ptx::mma_i8<2>(d_tmem, adesc + 256u * k, bdesc + 256u * k, idesc, (kb | k) != 0 ? 1u : 0u);
 #endif
-                        ptx::mma_i8<2>(d_tmem, adesc + 256u * k, bdesc + 256u * k, idesc, (kb | k) != 0 ? 1u : 0u);
-                    ptx::mma_commit_cg2(bar_empty + 8 * stage, 3);
+                        ptx::mma_commit_cg2(bar_empty + 8 * stage, 3);
+                    }
+                    __syncwarp();
                     if (++stage == S) { stage = 0; phase ^= 1; }
                 }
-                ptx::mma_commit_cg2(bar_tfull + 8 * buf, 3);
-                // every operand load of this tile has landed in shared memory (observed through the full barriers, so a
-                // relaxed count is enough): its ring slab may be recycled
-                ptx::red_relaxed_add_u64(p.done + w / p.tiles_per_chan, 1ull);
+                if (lane == 0) {
+                    ptx::mma_commit_cg2(bar_tfull + 8 * buf, 3);
+                    // every operand load of this tile has landed in shared memory (observed through the full
+                    // barriers, so a relaxed count is enough): its ring slab may be recycled
+                    ptx::red_relaxed_add_u64(p.done + tl.c, 1ull);
+                }
+                __syncwarp();
             }
         }
     } else if (warp >= 4 && warp < 8) {
@@ -227,11 +264,11 @@ xcorr_pair_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
         for (uint32_t it = 0;; ++it) {
             const long long w = ring.get<true>(it, lane);
             if (w < 0) break;
-            const int c = static_cast<int>(w / p.tiles_per_chan);
-            const PrTile tl = tiles[w % p.tiles_per_chan];
+            const PrWhere tl = pr_decode(w, p.tiles_per_chan);
+            const int c = tl.c;
             const uint32_t buf = it & 1, bphase = (it >> 1) & 1;
-            const int i0 = PR_BLK * tl.row_blk + 64 * static_cast<int>(rank) + 16 * wq;  // first input row of this warp
-            const int j0 = PR_BLK * tl.col_blk;
+            const int i0 = PR_BLK * tl.R + 64 * static_cast<int>(rank) + 16 * wq;  // first input row of this warp
+            const int j0 = PR_BLK * tl.Cb;
             // 64-column chunks that reach the diagonal or lie below it (i0 >= j0 always: Cb <= R)
             int nchunk = (i0 + 15 - j0) / TC_CJ + 1;
             nchunk = nchunk > 2 ? 2 : nchunk;
