@@ -344,11 +344,23 @@ def main():
     hbm["frac"] = hbm["achieved"] / hbm["peak"]
     main_r, alt_r = (tensor, hbm) if tensor["frac"] >= hbm["frac"] else (hbm, tensor)
     roofline = dict(main_r)
+    # DRAM traffic of the same kernel on the same workload from the committed ncu capture (profiles/), per launch
     roofline["traffic"] = None
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            tr = json.load(f).get(cfg.name)
+        if tr and args.algo == "tcgen05":
+            roofline["traffic"] = tr["dram_bytes_per_launch"]
+            roofline["traffic_source"] = tr["source"]
+    except (OSError, ValueError, KeyError):
+        pass
     roofline["peak_source"] = "%s (%s; int8 = 2 x bf16 %s)" % (
         peaks["source"], "MEASURED_PEAKS.json" if peaks["source"] == "measured" else "B200_PROFILING.md fallback",
         "sustained" if long_region else "burst")
-    roofline["kernel"] = "xcorr_tcgen05_kernel" if args.algo == "tcgen05" else "xcorr_simt_kernel"
+    roofline["kernel"] = ("xcorr_simt_kernel" if args.algo != "tcgen05" else
+                          "xcorr_pair_kernel" if cfg.ninputs > 64 else "xcorr_tcgen05_kernel")
+    # context: tcgen05.mma kind::i8 issue-rate probe on this pool (profiles/round1.md): 8192 MAC/clk/SM -> 4.6 POPS at 1.9 GHz
+    roofline["int8_mma_probe_peak_tops"] = 4610.0
     roofline["launch_ms"] = launch_ms
     roofline["algorithmic_ops_per_launch"] = ops_launch
     roofline["algorithmic_bytes_per_launch"] = bytes_launch

@@ -189,7 +189,6 @@ __device__ __forceinline__ void tc_epilogue_chunk(const TcParams& p, uint32_t la
     const int sgn = par ? -1 : 1;
     const uint32_t krow = lane >> 1;
     const uint32_t wr_off = (krow ^ ((krow >> 1) & 1)) * TC_STG_PITCH + 4 * par;
-    const uint32_t own_off = (lane ^ ((lane >> 1) & 1)) * TC_STG_PITCH;  // lanes 0..15: slot of row `lane`
     // the bulk group that read this staging buffer two chunks ago must be done with it
     if (lane < 16) ptx::bulk_wait_read<1>();
     __syncwarp();
@@ -226,12 +225,37 @@ __device__ __forceinline__ void tc_epilogue_chunk(const TcParams& p, uint32_t la
             if (REMOTE_RELEASE) ptx::mbar_arrive_cluster_addr(release_bar); else ptx::mbar_arrive(release_bar);
         }
     }
-    ptx::fence_proxy_async_smem();  // staging writes -> visible to the bulk-copy engine
     __syncwarp();
 #ifdef BFX_PROBE_NO_STORE
     return;
 #endif
+#ifdef BFX_EPI_DIRECT
+    // (alternative kept for measurement: profiles/round1.md) Write-out, coalesced: for each of the 16 rows the warp moves 2 x 32 consecutive visibilities (256 B per
+    // instruction) from the staging row to the packed triangle: plain 8-byte stores (accumulate = 0) or two
+    // 32-bit reductions performed at the L2 (accumulate != 0; the old values never travel to the SM).
+#pragma unroll 4
+    for (int r = 0; r < 16; ++r) {
+        const int i_row = i0 + r;
+        int n = i_row + 1 - jb;       // row i holds columns j <= i only (S2 masking of diagonal tiles)
+        if (i_row >= p.ninputs) n = 0;
+        int32_t* const g0 = out_c + 2 * (static_cast<long long>(i_row) * (i_row + 1) / 2 + jb);
+        const uint32_t s0 = stg_buf + (r ^ ((r >> 1) & 1)) * TC_STG_PITCH;
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const int j = static_cast<int>(lane) + 32 * h;
+            if (j < n) {
+                int2 v;
+                asm volatile("ld.shared.v2.s32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(s0 + 8 * j));
+                if (p.accumulate) ptx::red_add_global_v2(g0 + 2 * j, v); else ptx::st_global_v2(g0 + 2 * j, v);
+            }
+        }
+    }
+    __syncwarp();
+#else
+    ptx::fence_proxy_async_smem();  // staging writes -> visible to the bulk-copy engine
+    __syncwarp();
     if (lane < 16) {
+        const uint32_t own_off = (lane ^ ((lane >> 1) & 1)) * TC_STG_PITCH;  // lanes 0..15: slot of row `lane`
         const int i_own = i0 + static_cast<int>(lane);
         int n = i_own + 1 - jb;       // row i holds columns j <= i only (S2 masking of diagonal tiles)
         n = n > TC_CJ ? TC_CJ : n;
@@ -259,6 +283,7 @@ __device__ __forceinline__ void tc_epilogue_chunk(const TcParams& p, uint32_t la
         }
         ptx::bulk_commit();
     }
+#endif
 }
 
 // ===================== relayout warps (S1: unpack-and-transpose, span -> ring z) =====================
