@@ -278,6 +278,61 @@ __device__ __forceinline__ void red_add_global_v2(int32_t* p, int2 v)
     asm volatile("red.global.add.u32 [%0], %1;\n\tred.global.add.u32 [%0+4], %2;" ::"l"(p), "r"(v.x), "r"(v.y) : "memory");
 }
 
+// ---- L2 eviction policies ----------------------------------------------------------------------
+__device__ __forceinline__ uint64_t policy_evict_last()
+{
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+
+__device__ __forceinline__ uint64_t policy_evict_first()
+{
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+
+__device__ __forceinline__ uint4 ld_global_stream_v4_hint(const uint8_t* p, uint64_t pol)
+{
+    uint4 v;
+    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.v4.u32 {%0, %1, %2, %3}, [%4], %5;"
+                 : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w)
+                 : "l"(p), "l"(pol));
+    return v;
+}
+
+__device__ __forceinline__ void st_global_v4_hint(uint8_t* p, uint4 v, uint64_t pol)
+{
+    asm volatile("st.global.L2::cache_hint.v4.u32 [%0], {%1, %2, %3, %4}, %5;" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w),
+                 "l"(pol)
+                 : "memory");
+}
+
+__device__ __forceinline__ void tma_load_3d_cg2_hint(uint32_t dst, const CUtensorMap* m, uint32_t bar, int x, int y, int z,
+                                                     uint64_t pol)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.cta_group::2.L2::cache_hint [%0], "
+        "[%1, {%3, %4, %5}], [%2], %6;" ::"r"(dst),
+        "l"(reinterpret_cast<uint64_t>(m)), "r"(bar), "r"(x), "r"(y), "r"(z), "l"(pol)
+        : "memory");
+}
+
+__device__ __forceinline__ void bulk_store_hint(void* gdst, uint32_t ssrc, uint32_t bytes, uint64_t pol)
+{
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;" ::"l"(gdst), "r"(ssrc),
+                 "r"(bytes), "l"(pol)
+                 : "memory");
+}
+
+__device__ __forceinline__ void bulk_reduce_add_s32_hint(void* gdst, uint32_t ssrc, uint32_t bytes, uint64_t pol)
+{
+    asm volatile("cp.reduce.async.bulk.global.shared::cta.bulk_group.L2::cache_hint.add.s32 [%0], [%1], %2, %3;" ::"l"(gdst),
+                 "r"(ssrc), "r"(bytes), "l"(pol)
+                 : "memory");
+}
+
 // ---- inter-CTA flags ---------------------------------------------------------------------------
 __device__ __forceinline__ unsigned long long ld_acquire_u64(const unsigned long long* p)
 {

@@ -148,6 +148,9 @@ xcorr_pair_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
         // ===================== TMA producer (+ tile scheduler in the leader) =====================
         uint32_t stage = 0, phase = 0;
         int ready_chan = -1;
+#ifdef BFX_L2_HINTS
+        const uint64_t pol_last = ptx::policy_evict_last();  // ring slabs are re-read by every tile of the channel
+#endif
         // the leader draws tile n + 1 from the global counter before it loads tile n: the atomic's round trip
         // (and everything the other roles do on receiving an index) overlaps the loads of the current tile
         unsigned long long w_next = 0;
@@ -206,8 +209,13 @@ xcorr_pair_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
                     const uint32_t dst = op_base + stage * PR_STAGE_BYTES;
                     const uint32_t fullb = lead_full + 8 * stage;
                     const int t0 = kb * TC_KT;
+#ifdef BFX_L2_HINTS
+                    ptx::tma_load_3d_cg2_hint(dst, &tmap, fullb, xa, cs, t0, pol_last);
+                    if (!diag) ptx::tma_load_3d_cg2_hint(dst + TC_BOX_BYTES, &tmap, fullb, xb, cs, t0, pol_last);
+#else
                     ptx::tma_load_3d_cg2(dst, &tmap, fullb, xa, cs, t0);
                     if (!diag) ptx::tma_load_3d_cg2(dst + TC_BOX_BYTES, &tmap, fullb, xb, cs, t0);
+#endif
 #endif
                 }
                 __syncwarp();

@@ -34,6 +34,10 @@ namespace bfx {
 // ---- tile geometry ----------------------------------------------------------------------------
 constexpr int TC_BM_IN = 64;    // inputs per A tile  -> UMMA M = 128 real rows
 constexpr int TC_BN_IN = 128;   // inputs per B tile  -> UMMA N = 256 real columns (two 64-input boxes)
+// L2 eviction hints (A/B measured, profiles/round1.md): ring slabs evict_last, span reads and visibility writes evict_first
+#ifndef BFX_NO_L2_HINTS
+#define BFX_L2_HINTS 1
+#endif
 #ifndef BFX_KT
 #define BFX_KT 128
 #endif
@@ -272,8 +276,14 @@ __device__ __forceinline__ void tc_epilogue_chunk(const TcParams& p, uint32_t la
                 if (p.accumulate) ptx::red_add_global_v2(g0, v); else ptx::st_global_v2(g0, v);
             }
             if (nbulk > 0) {
+#ifdef BFX_L2_HINTS
+                // the visibilities stream through the L2 once per span: let them go first, the S1 ring should stay
+                if (p.accumulate) ptx::bulk_reduce_add_s32_hint(g0 + 2 * head, s0 + 8 * head, 8u * nbulk, ptx::policy_evict_first());
+                else ptx::bulk_store_hint(g0 + 2 * head, s0 + 8 * head, 8u * nbulk, ptx::policy_evict_first());
+#else
                 if (p.accumulate) ptx::bulk_reduce_add_s32(g0 + 2 * head, s0 + 8 * head, 8u * nbulk);
                 else ptx::bulk_store(g0 + 2 * head, s0 + 8 * head, 8u * nbulk);
+#endif
             }
             if (head + nbulk < n) {
                 int2 v;
@@ -299,6 +309,9 @@ __device__ __forceinline__ void tc_relayout_role(const TcParams& p, uint32_t lan
     // 16-byte stores to the channel's slab.  Each warp works on its own units.
     const long long src_pitch = static_cast<long long>(p.nchan) * p.row_in;
     const int row_out = 2 * p.ninputs;
+#ifdef BFX_L2_HINTS
+    const uint64_t pol_first = ptx::policy_evict_first(), pol_last = ptx::policy_evict_last();  // span: once; ring: keep
+#endif
     auto do_unit = [&](int cc, int u) {
         if (cc >= p.ring_w) {
             // the slab is still owned by channel cc - ring_w until all of its tiles have loaded their operands
