@@ -154,6 +154,7 @@ template <bool CI4>
 int launch_tcgen05(bfXcorr p, const void* in, void* out, int accumulate, cudaStream_t stream)
 {
     const bool fused = p->d_z != nullptr;
+    const bool pair = p->d_pair_tiles != nullptr;
     const OperandSource src = fused ? ring_source(p) : direct_source(p, in);
     CUtensorMap tmap;
     // operand boxes: 64 inputs x 1 channel x TC_KT samples (128 bytes of int8 pairs, or 64 raw ci4 bytes)
@@ -179,13 +180,18 @@ int launch_tcgen05(bfXcorr p, const void* in, void* out, int accumulate, cudaStr
         prm.row_in = static_cast<int>(p->ninputs * bytes_per_sample(p->dtype));
         prm.ring_w = p->ring_w;
         prm.rl_nx = (prm.row_in + bfx::RL_XBYTES - 1) / bfx::RL_XBYTES;
-        prm.rl_units = prm.rl_nx * ((p->ntime + bfx::RL_ROWS - 1) / bfx::RL_ROWS);
+        // a unit = rl_rows samples x one row piece of <= 1 KiB: about 8 KiB, one round of 16 loads per lane
+        const int piece = prm.row_in < bfx::RL_XBYTES ? prm.row_in : bfx::RL_XBYTES;
+        int rows = bfx::RL_ROWS * bfx::RL_XBYTES / piece;
+        if (rows > 256) rows = 256;
+        prm.rl_rows = rows;
+        prm.rl_units = prm.rl_nx * ((p->ntime + rows - 1) / rows);
         prm.ready = p->d_flags;
         prm.done = p->d_flags + p->nchan;
         prm.epoch = ++p->epoch;
     }
     cudaError_t e = cudaSuccess;
-    if (fused) {
+    if (pair) {
         // one cluster of two CTAs per tile in flight
         prm.pair_tiles = p->d_pair_tiles;
         long long pairs = p->num_sms / 2;

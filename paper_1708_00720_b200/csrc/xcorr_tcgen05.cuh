@@ -89,7 +89,8 @@ struct TcParams {
     uint8_t* z;
     int row_in;             // bytes of one (t, c) row of the span
     int ring_w;
-    int rl_nx, rl_units;    // 1 KiB pieces per row; relayout units per channel = rl_nx * ceil(ntime / RL_ROWS)
+    int rl_nx, rl_units;    // 1 KiB pieces per row; relayout units per channel = rl_nx * ceil(ntime / rl_rows)
+    int rl_rows;            // samples per relayout unit (a unit is about 8 KiB of span)
     unsigned long long* ready;
     unsigned long long* done;
     unsigned long long epoch;  // 1, 2, ... : launch number of this plan
@@ -325,9 +326,9 @@ __device__ __forceinline__ void tc_relayout_role(const TcParams& p, uint32_t lan
             }
             __syncwarp();
         }
-        const int t0 = (u / p.rl_nx) * RL_ROWS;
+        const int t0 = (u / p.rl_nx) * p.rl_rows;
         const int xb0 = (u % p.rl_nx) * RL_XBYTES;
-        const int nt = min(RL_ROWS, p.ntime - t0);
+        const int nt = min(p.rl_rows, p.ntime - t0);
         const int nv = min(RL_XBYTES, p.row_in - xb0) >> 4;  // 16-byte vectors per row piece
         const int total = nt * nv;
         const int nv_shift = (nv & (nv - 1)) == 0 ? 31 - __clz(nv) : -1;  // rows are usually 64 vectors: avoid the division
