@@ -11,6 +11,7 @@
 
 #include "../../include/bfxcorr.h"
 #include "xcorr_simt.cuh"
+#include "xcorr_few.cuh"
 #include "xcorr_pair.cuh"
 #include "xcorr_tcgen05.cuh"
 
@@ -135,11 +136,11 @@ OperandSource ring_source(bfXcorr p)
 }
 
 int encode_map(bfXcorr p, CUtensorMap* m, CUtensorMapDataType type, const OperandSource& src, unsigned elem_bytes,
-               unsigned box_elems, CUtensorMapSwizzle swz, int nchan_src)
+               unsigned box_elems, CUtensorMapSwizzle swz, int nchan_src, unsigned box_chan = 1, unsigned box_rows = bfx::TC_KT)
 {
     const cuuint64_t dims[3] = {src.row / elem_bytes, static_cast<cuuint64_t>(nchan_src), static_cast<cuuint64_t>(p->ntime)};
     const cuuint64_t strides[2] = {src.chan_stride, src.time_stride};
-    const cuuint32_t box[3] = {box_elems, 1u, static_cast<cuuint32_t>(bfx::TC_KT)};
+    const cuuint32_t box[3] = {box_elems, box_chan, box_rows};
     const cuuint32_t estr[3] = {1u, 1u, 1u};
     const CUresult r = p->encode(m, type, 3, const_cast<void*>(src.base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                                  swz, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
@@ -155,11 +156,15 @@ int launch_tcgen05(bfXcorr p, const void* in, void* out, int accumulate, cudaStr
 {
     const bool fused = p->d_z != nullptr;
     const bool pair = p->d_pair_tiles != nullptr;
+    const bool few = CI4 && !pair;  // ci4, ninputs <= 64: xcorr_few.cuh, FW_NC channels per CTA tile
     const OperandSource src = fused ? ring_source(p) : direct_source(p, in);
     CUtensorMap tmap;
-    // operand boxes: 64 inputs x 1 channel x TC_KT samples (128 bytes of int8 pairs, or 64 raw ci4 bytes)
-    const int st = encode_map(p, &tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, src, 1, CI4 ? 64u : 128u,
-                              CI4 ? CU_TENSOR_MAP_SWIZZLE_NONE : CU_TENSOR_MAP_SWIZZLE_128B, fused ? p->ring_w : p->nchan);
+    // operand boxes: 64 inputs x 1 channel x TC_KT samples (128 bytes of int8 pairs); few-input ci4: whole raw rows of
+    // FW_NC adjacent channels x FW_KT samples
+    const int st = few ? encode_map(p, &tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, src, 1, static_cast<unsigned>(src.row),
+                                    CU_TENSOR_MAP_SWIZZLE_NONE, p->nchan, bfx::FW_NC, bfx::FW_KT)
+                       : encode_map(p, &tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, src, 1, CI4 ? 64u : 128u,
+                                    CI4 ? CU_TENSOR_MAP_SWIZZLE_NONE : CU_TENSOR_MAP_SWIZZLE_128B, fused ? p->ring_w : p->nchan);
     if (st != BF_XCORR_OK) return st;
     TcParams prm;
     std::memset(&prm, 0, sizeof(prm));
@@ -210,6 +215,11 @@ int launch_tcgen05(bfXcorr p, const void* in, void* out, int accumulate, cudaStr
         cfg.attrs = &attr;
         cfg.numAttrs = 1;
         e = cudaLaunchKernelEx(&cfg, bfx::xcorr_pair_kernel, tmap, prm);
+    } else if (few) {
+        prm.ntiles = (p->nchan + bfx::FW_NC - 1) / bfx::FW_NC;
+        prm.row_in = static_cast<int>(src.row);
+        const long long want = prm.ntiles < p->num_sms ? prm.ntiles : p->num_sms;
+        bfx::xcorr_few_kernel<<<dim3(static_cast<unsigned>(want)), bfx::FW_THREADS, bfx::FW_SMEM_BYTES, stream>>>(tmap, prm);
     } else {
         const long long want = prm.ntiles < p->num_sms ? prm.ntiles : p->num_sms;
         const dim3 grid(static_cast<unsigned>(want));
@@ -311,6 +321,8 @@ int bfXcorrCreate(bfXcorr* plan, int ninputs, int nchan, int ntime, int dtype)
         if (e == cudaSuccess) e = cudaMalloc(reinterpret_cast<void**>(&p->d_flags), 2ull * nchan * sizeof(unsigned long long));
         if (e == cudaSuccess) e = cudaMemset(p->d_flags, 0, 2ull * nchan * sizeof(unsigned long long));
     }
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(bfx::xcorr_few_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bfx::FW_SMEM_BYTES);
     if (e == cudaSuccess)
         e = cudaFuncSetAttribute(bfx::xcorr_pair_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bfx::PR_SMEM_BYTES);
     if (e == cudaSuccess)
