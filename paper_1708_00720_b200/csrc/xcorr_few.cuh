@@ -6,9 +6,9 @@
 // TMA box row is a contiguous run of 4 x 64 bytes and the translations per byte drop fourfold; the four
 // 128-lane x 128-column accumulators fill the CTA's 512 TMEM columns.
 //
-// Roles (384 threads): warp 0 TMA producer (raw nibble bytes, box {row bytes, 4 channels, FW_KT samples}),
+// Roles (512 threads): warp 0 TMA producer (raw nibble bytes, box {row bytes, 4 channels, FW_KT samples}),
 // warp 1 MMA issuer (per channel: A = B = the channel's int8 tile, M = 128, N = 128), warp 2 TMEM allocator,
-// warps 4..7 epilogue (tc_epilogue_chunk, one 64-visibility chunk per channel), warps 8..11 unpack: raw bytes ->
+// warps 4..7 epilogue (tc_epilogue_chunk, one 64-visibility chunk per channel), warps 8..15 unpack: raw bytes ->
 // 128B-swizzled int8 tiles (nibble << 4; the 16 x 16 scale is shifted out exactly in the epilogue).
 #pragma once
 #include "xcorr_tcgen05.cuh"
@@ -21,7 +21,8 @@ constexpr int FW_RAW_STAGES = 3, FW_OP_STAGES = 3;
 constexpr int FW_RAW_STAGE_BYTES = FW_KT * FW_NC * 64;    // [t][c][<= 64 B]
 constexpr int FW_OP_TILE_BYTES = FW_KT * 128;             // one channel: [t][128 B] swizzled
 constexpr int FW_OP_STAGE_BYTES = FW_NC * FW_OP_TILE_BYTES;
-constexpr int FW_THREADS = 384;
+constexpr int FW_UNPACK_WARPS = 8;
+constexpr int FW_THREADS = 256 + 32 * FW_UNPACK_WARPS;
 constexpr int FW_SMEM_BYTES = 1024 + FW_RAW_STAGES * FW_RAW_STAGE_BYTES + FW_OP_STAGES * FW_OP_STAGE_BYTES + TC_STG_BYTES + 512;
 
 __global__ void __launch_bounds__(FW_THREADS, 1)
@@ -34,10 +35,10 @@ xcorr_few_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
     const uint32_t raw_base = op_base + S * FW_OP_STAGE_BYTES;
     const uint32_t stg_base = raw_base + R * FW_RAW_STAGE_BYTES;
     const uint32_t bar_base = stg_base + TC_STG_BYTES;
-    const uint32_t bar_full = bar_base;               // [S] int8 tiles written by the 4 unpack warps
+    const uint32_t bar_full = bar_base;               // [S] int8 tiles written by the unpack warps
     const uint32_t bar_empty = bar_full + 8 * S;      // [S] MMAs reading the stage have completed
     const uint32_t bar_rfull = bar_empty + 8 * S;     // [R] raw bytes landed
-    const uint32_t bar_rempty = bar_rfull + 8 * R;    // [R] raw bytes consumed by the 4 unpack warps
+    const uint32_t bar_rempty = bar_rfull + 8 * R;    // [R] raw bytes consumed by the unpack warps
     const uint32_t bar_tfull = bar_rempty + 8 * R;    // accumulators complete
     const uint32_t bar_tempty = bar_tfull + 8;        // accumulators drained by the 4 epilogue warps
     const uint32_t tmem_slot = bar_tempty + 8;
@@ -55,18 +56,18 @@ xcorr_few_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
     if (warp == 0 && lane == 0) {
         ptx::prefetch_tensormap(&tmap);
         for (int s = 0; s < S; ++s) {
-            ptx::mbar_init(bar_full + 8 * s, 4);
+            ptx::mbar_init(bar_full + 8 * s, FW_UNPACK_WARPS);
             ptx::mbar_init(bar_empty + 8 * s, 1);
         }
         for (int s = 0; s < R; ++s) {
             ptx::mbar_init(bar_rfull + 8 * s, 1);
-            ptx::mbar_init(bar_rempty + 8 * s, 4);
+            ptx::mbar_init(bar_rempty + 8 * s, FW_UNPACK_WARPS);
         }
         ptx::mbar_init(bar_tfull, 1);
         ptx::mbar_init(bar_tempty, 4);
         for (int s = 0; s < TC_RING; ++s) {
             ptx::mbar_init(bar_sfull + 8 * s, 1);
-            ptx::mbar_init(bar_sempty + 8 * s, 9);  // MMA issuer + 4 epilogue warps + 4 unpack warps
+            ptx::mbar_init(bar_sempty + 8 * s, 5 + FW_UNPACK_WARPS);  // MMA issuer + 4 epilogue warps + unpack warps
         }
         ptx::fence_barrier_init();
     }
@@ -177,8 +178,8 @@ xcorr_few_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
         // ===================== unpack warps (S1): raw [t][c][row] nibble bytes -> per-channel int8 tiles =====================
         // int8 tile: [t][128 B], byte 2i = re_i << 4, byte 2i+1 = im_i << 4, 16-byte chunks XOR-swizzled by (t & 7)
         // exactly as TMA SWIZZLE_128B would have written them.
-        const int tid = (warp - 8) * 32 + static_cast<int>(lane);  // 0..127
-        const int qn = row >> 4;                                    // 16-byte chunks per raw row
+        const int uw = warp - 8, tl = static_cast<int>(lane >> 2), qc = static_cast<int>(lane & 3);
+        const int qn = row >> 4;                                    // 16-byte chunks per raw row (1..4)
         uint32_t rstage = 0, rphase = 0, ostage = 0, ophase = 0;
         for (uint32_t it = 0;; ++it) {
             const long long w = ring.get<true>(it, lane);
@@ -188,27 +189,32 @@ xcorr_few_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
                 ptx::mbar_wait(bar_empty + 8 * ostage, ophase ^ 1);
                 const uint32_t rsrc = raw_base + rstage * FW_RAW_STAGE_BYTES;
                 const uint32_t odst = op_base + ostage * FW_OP_STAGE_BYTES;
-                const int ntask = FW_KT * FW_NC * qn;
-                for (int task = tid; task < ntask; task += 128) {
-                    const int qc = task % qn, tc = task / qn;   // tc = t * FW_NC + ch
-                    const int ch = tc % FW_NC, t = tc / FW_NC;
-                    uint32_t wv[4];
-                    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
-                                 : "=r"(wv[0]), "=r"(wv[1]), "=r"(wv[2]), "=r"(wv[3])
-                                 : "r"(rsrc + tc * row + qc * 16));
-                    uint32_t o[8];
+                // lane -> (row t, 16-byte chunk qc) of one channel: a quarter-warp writes 2 rows x 4 chunks of a
+                // swizzled tile, which touches every bank once; no divisions on the way
 #pragma unroll
-                    for (int u = 0; u < 4; ++u) {
-                        const uint32_t hi = wv[u] & 0xF0F0F0F0u;          // 4 x (re << 4)
-                        const uint32_t lo = (wv[u] << 4) & 0xF0F0F0F0u;   // 4 x (im << 4)
-                        o[2 * u] = __byte_perm(hi, lo, 0x5140);           // re0 im0 re1 im1
-                        o[2 * u + 1] = __byte_perm(hi, lo, 0x7362);       // re2 im2 re3 im3
+                for (int ch = 0; ch < FW_NC; ++ch) {
+#pragma unroll
+                    for (int t = uw * 8 + tl; t < FW_KT; t += 8 * FW_UNPACK_WARPS) {
+                        if (qc < qn) {
+                            uint32_t wv[4];
+                            asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
+                                         : "=r"(wv[0]), "=r"(wv[1]), "=r"(wv[2]), "=r"(wv[3])
+                                         : "r"(rsrc + (t * FW_NC + ch) * row + qc * 16));
+                            uint32_t o[8];
+#pragma unroll
+                            for (int u = 0; u < 4; ++u) {
+                                const uint32_t hi = wv[u] & 0xF0F0F0F0u;          // 4 x (re << 4)
+                                const uint32_t lo = (wv[u] << 4) & 0xF0F0F0F0u;   // 4 x (im << 4)
+                                o[2 * u] = __byte_perm(hi, lo, 0x5140);           // re0 im0 re1 im1
+                                o[2 * u + 1] = __byte_perm(hi, lo, 0x7362);       // re2 im2 re3 im3
+                            }
+                            const uint32_t rowa = odst + ch * FW_OP_TILE_BYTES + t * 128;
+                            const uint32_t a0 = rowa + static_cast<uint32_t>((2 * qc) ^ (t & 7)) * 16;
+                            const uint32_t a1 = rowa + static_cast<uint32_t>((2 * qc + 1) ^ (t & 7)) * 16;
+                            asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(a0), "r"(o[0]), "r"(o[1]), "r"(o[2]), "r"(o[3]) : "memory");
+                            asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(a1), "r"(o[4]), "r"(o[5]), "r"(o[6]), "r"(o[7]) : "memory");
+                        }
                     }
-                    const uint32_t rowa = odst + ch * FW_OP_TILE_BYTES + t * 128;
-                    const uint32_t a0 = rowa + static_cast<uint32_t>((2 * qc) ^ (t & 7)) * 16;
-                    const uint32_t a1 = rowa + static_cast<uint32_t>((2 * qc + 1) ^ (t & 7)) * 16;
-                    asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(a0), "r"(o[0]), "r"(o[1]), "r"(o[2]), "r"(o[3]) : "memory");
-                    asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(a1), "r"(o[4]), "r"(o[5]), "r"(o[6]), "r"(o[7]) : "memory");
                 }
                 ptx::fence_proxy_async_smem();  // generic-proxy stores -> visible to the tensor core (async proxy)
                 __syncwarp();
