@@ -4,7 +4,6 @@
 #include <cstdio>
 #include <cstring>
 #include <new>
-#include <vector>
 
 #include <cuda.h>
 #include <cuda_runtime.h>
@@ -13,14 +12,11 @@
 #include "xcorr_simt.cuh"
 #include "xcorr_few.cuh"
 #include "xcorr_pair.cuh"
-#include "xcorr_tcgen05.cuh"
+#include "xcorr_common.cuh"
 
 namespace {
 
-using bfx::TcCfg;
 using bfx::TcParams;
-using bfx::TcTile;
-using bfx::PrTile;
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
@@ -39,8 +35,7 @@ struct bfXcorr_impl {
     int last_cuda_error;
     int last_launch_count;
     // S2: lower-triangle tile table (device copy) for the tcgen05 kernel
-    TcTile* d_tiles;      // 1-CTA kernel (ninputs <= 64)
-    PrTile* d_pair_tiles; // CTA-pair kernel (ninputs > 64)
+    bool pair;            // ninputs > 64: CTA-pair kernel with fused S1; else the few-input kernel
     int tiles_per_chan;
     unsigned long long* d_sched;  // dynamic tile scheduler state, re-armed by the kernel itself
     EncodeTiledFn encode;
@@ -75,41 +70,6 @@ unsigned long long output_bytes(bfXcorr p)
 {
     const unsigned long long n = p->ninputs;
     return static_cast<unsigned long long>(p->nchan) * (n * (n + 1) / 2) * 8ull;
-}
-
-// S2: enumerate only the tiles that touch the lower triangle.  Row blocks are 64
-// inputs (UMMA M = 128 real rows), column blocks 128 inputs (UMMA N = 256); a tile whose second 64-input
-// column half lies wholly above the diagonal (or beyond N) is issued with N = 128.
-std::vector<TcTile> build_tiles(int ninputs)
-{
-    std::vector<TcTile> tiles;
-    const int nrb = (ninputs + bfx::TC_BM_IN - 1) / bfx::TC_BM_IN;
-    for (int r = 0; r < nrb; ++r) {
-        const int i0 = r * bfx::TC_BM_IN;
-        const int i_last = (i0 + bfx::TC_BM_IN < ninputs ? i0 + bfx::TC_BM_IN : ninputs) - 1;
-        for (int cb = 0; cb * bfx::TC_BN_IN <= i_last; ++cb) {
-            const int j0 = cb * bfx::TC_BN_IN;
-            TcTile t;
-            t.row_blk = static_cast<int16_t>(r);
-            t.col_blk = static_cast<int16_t>(cb);
-            t.nbox = static_cast<int8_t>((j0 + 64 <= i_last) ? 2 : 1);
-            const int d = (i0 - j0) / 64;
-            t.a_alias = static_cast<int8_t>((i0 >= j0 && d < t.nbox) ? d : -1);
-            t.pad = 0;
-            tiles.push_back(t);
-        }
-    }
-    return tiles;
-}
-
-// S2 for the CTA-pair kernel: 128 x 128-input tiles on or below the diagonal, row-major.
-std::vector<PrTile> build_pair_tiles(int ninputs)
-{
-    std::vector<PrTile> tiles;
-    const int nb = (ninputs + bfx::PR_BLK - 1) / bfx::PR_BLK;
-    for (int r = 0; r < nb; ++r)
-        for (int cb = 0; cb <= r; ++cb) tiles.push_back(PrTile{static_cast<int16_t>(r), static_cast<int16_t>(cb)});
-    return tiles;
 }
 
 // Where the tensor-core kernel reads its operands from: the caller's span x[t][c][...] itself (direct), or the
@@ -155,8 +115,8 @@ template <bool CI4>
 int launch_tcgen05(bfXcorr p, const void* in, void* out, int accumulate, cudaStream_t stream)
 {
     const bool fused = p->d_z != nullptr;
-    const bool pair = p->d_pair_tiles != nullptr;
-    const bool few = CI4 && !pair;  // ci4, ninputs <= 64: xcorr_few.cuh, FW_NC channels per CTA tile
+    const bool pair = p->pair;
+    const bool few = !pair;  // ninputs <= 64: xcorr_few.cuh, FW_NC channels per CTA tile
     const OperandSource src = fused ? ring_source(p) : direct_source(p, in);
     CUtensorMap tmap;
     // operand boxes: 64 inputs x 1 channel x TC_KT samples (128 bytes of int8 pairs); few-input ci4: whole raw rows of
@@ -169,7 +129,6 @@ int launch_tcgen05(bfXcorr p, const void* in, void* out, int accumulate, cudaStr
     TcParams prm;
     std::memset(&prm, 0, sizeof(prm));
     prm.out = static_cast<int32_t*>(out);
-    prm.tiles = p->d_tiles;
     prm.ninputs = p->ninputs;
     prm.nchan = p->nchan;
     prm.ntime = p->ntime;
@@ -178,7 +137,6 @@ int launch_tcgen05(bfXcorr p, const void* in, void* out, int accumulate, cudaStr
     prm.accumulate = accumulate ? 1 : 0;
     prm.sched = p->d_sched;
     if (fused) {
-        prm.rl_enabled = 1;
         prm.rl_ci4 = p->dtype == BF_XCORR_CI4 ? 1 : 0;
         prm.x = static_cast<const uint8_t*>(in);
         prm.z = p->d_z;
@@ -198,7 +156,6 @@ int launch_tcgen05(bfXcorr p, const void* in, void* out, int accumulate, cudaStr
     cudaError_t e = cudaSuccess;
     if (pair) {
         // one cluster of two CTAs per tile in flight
-        prm.pair_tiles = p->d_pair_tiles;
         long long pairs = p->num_sms / 2;
         if (prm.ntiles < pairs) pairs = prm.ntiles;
         cudaLaunchConfig_t cfg;
@@ -219,11 +176,7 @@ int launch_tcgen05(bfXcorr p, const void* in, void* out, int accumulate, cudaStr
         prm.ntiles = (p->nchan + bfx::FW_NC - 1) / bfx::FW_NC;
         prm.row_in = static_cast<int>(src.row);
         const long long want = prm.ntiles < p->num_sms ? prm.ntiles : p->num_sms;
-        bfx::xcorr_few_kernel<<<dim3(static_cast<unsigned>(want)), bfx::FW_THREADS, bfx::FW_SMEM_BYTES, stream>>>(tmap, prm);
-    } else {
-        const long long want = prm.ntiles < p->num_sms ? prm.ntiles : p->num_sms;
-        const dim3 grid(static_cast<unsigned>(want));
-        bfx::xcorr_tcgen05_kernel<CI4><<<grid, TcCfg<CI4>::kThreads, TcCfg<CI4>::kSmemBytes, stream>>>(tmap, prm);
+        bfx::xcorr_few_kernel<CI4><<<dim3(static_cast<unsigned>(want)), bfx::FW_THREADS, bfx::FwCfg<CI4>::kSmemBytes, stream>>>(tmap, prm);
     }
     if (e == cudaSuccess) e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(p, e);
@@ -289,19 +242,17 @@ int bfXcorrCreate(bfXcorr* plan, int ninputs, int nchan, int ntime, int dtype)
     }
     p->encode = reinterpret_cast<EncodeTiledFn>(fn);
 
-    const bool pair = ninputs > bfx::TC_BM_IN;  // more than one tile per channel: CTA pairs + fused S1
-    if (pair) {
-        const std::vector<PrTile> tiles = build_pair_tiles(ninputs);
-        p->tiles_per_chan = static_cast<int>(tiles.size());
-        e = cudaMalloc(reinterpret_cast<void**>(&p->d_pair_tiles), tiles.size() * sizeof(PrTile));
-        if (e == cudaSuccess)
-            e = cudaMemcpy(p->d_pair_tiles, tiles.data(), tiles.size() * sizeof(PrTile), cudaMemcpyHostToDevice);
-    } else {
-        const std::vector<TcTile> tiles = build_tiles(ninputs);
-        p->tiles_per_chan = static_cast<int>(tiles.size());
-        e = cudaMalloc(reinterpret_cast<void**>(&p->d_tiles), tiles.size() * sizeof(TcTile));
-        if (e == cudaSuccess) e = cudaMemcpy(p->d_tiles, tiles.data(), tiles.size() * sizeof(TcTile), cudaMemcpyHostToDevice);
+    // S2: tiles of a channel = 128 x 128-input blocks on or below the diagonal (xcorr_pair.cuh decodes the index);
+    // up to 64 inputs: a single 64 x 64 tile per channel (xcorr_few.cuh)
+    const bool pair = ninputs > 64;
+    p->pair = pair;
+    const int nblk = (ninputs + bfx::PR_BLK - 1) / bfx::PR_BLK;
+    p->tiles_per_chan = pair ? nblk * (nblk + 1) / 2 : 1;
+    if (pair && static_cast<unsigned long long>(p->tiles_per_chan) * nchan >= (1ull << 32)) {
+        delete p;
+        return BF_XCORR_UNSUPPORTED_SHAPE;
     }
+    e = cudaSuccess;
     if (e == cudaSuccess) e = cudaMalloc(reinterpret_cast<void**>(&p->d_sched), 4 * sizeof(unsigned long long));
     if (e == cudaSuccess) e = cudaMemset(p->d_sched, 0, 4 * sizeof(unsigned long long));
     // A channel whose tiles re-read its samples is first rewritten channel-major (xcorr_relayout.cuh); with a
@@ -322,19 +273,13 @@ int bfXcorrCreate(bfXcorr* plan, int ninputs, int nchan, int ntime, int dtype)
         if (e == cudaSuccess) e = cudaMemset(p->d_flags, 0, 2ull * nchan * sizeof(unsigned long long));
     }
     if (e == cudaSuccess)
-        e = cudaFuncSetAttribute(bfx::xcorr_few_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bfx::FW_SMEM_BYTES);
+        e = cudaFuncSetAttribute(bfx::xcorr_few_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bfx::FwCfg<true>::kSmemBytes);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(bfx::xcorr_few_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bfx::FwCfg<false>::kSmemBytes);
     if (e == cudaSuccess)
         e = cudaFuncSetAttribute(bfx::xcorr_pair_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bfx::PR_SMEM_BYTES);
-    if (e == cudaSuccess)
-        e = cudaFuncSetAttribute(bfx::xcorr_tcgen05_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 TcCfg<false>::kSmemBytes);
-    if (e == cudaSuccess)
-        e = cudaFuncSetAttribute(bfx::xcorr_tcgen05_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 TcCfg<true>::kSmemBytes);
     if (e != cudaSuccess) {
         const int st = cuda_fail(nullptr, e);
-        if (p->d_tiles) cudaFree(p->d_tiles);
-        if (p->d_pair_tiles) cudaFree(p->d_pair_tiles);
         if (p->d_sched) cudaFree(p->d_sched);
         if (p->d_z) cudaFree(p->d_z);
         if (p->d_flags) cudaFree(p->d_flags);
@@ -382,8 +327,6 @@ int bfXcorrExecuteHost(bfXcorr plan, const void* in_host, void* out_dev, void* o
 int bfXcorrDestroy(bfXcorr plan)
 {
     if (!valid(plan)) return BF_XCORR_INVALID_HANDLE;
-    if (plan->d_tiles) cudaFree(plan->d_tiles);
-    if (plan->d_pair_tiles) cudaFree(plan->d_pair_tiles);
     if (plan->d_sched) cudaFree(plan->d_sched);
     if (plan->d_stage_in) cudaFree(plan->d_stage_in);
     if (plan->d_z) cudaFree(plan->d_z);

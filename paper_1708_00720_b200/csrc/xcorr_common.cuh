@@ -1,4 +1,5 @@
-// xcorr_tcgen05.cuh -- the X-engine hot path on sm_100a tensor cores (BF_XCORR_ALGO_TCGEN05).
+// xcorr_common.cuh -- pieces shared by the tensor-core kernels of the X-engine (xcorr_pair.cuh, xcorr_few.cuh):
+// kernel parameters, UMMA descriptors, the tile-index ring, the S4 epilogue chunk and the S1 relayout role.
 //
 // Real embedding: a span row x[t][c][0..N) of ci8 samples is, byte for byte, the
 // int8 row z[t][0..2N) with z[2i] = re_i, z[2i+1] = im_i.  The real Gram matrix
@@ -7,23 +8,14 @@
 //     Re V[i][j] = G[2i][2j]   + G[2i+1][2j+1]
 //     Im V[i][j] = G[2i+1][2j] - G[2i][2j+1]
 // so no operand negation is needed (kind::i8 has none) and the extreme code -128 stays exact.
-// z is "MN-major" for both MMA operands (the time axis is K), so the raw span is the operand: a TMA box
-// {128 bytes of m, 1 channel, KT samples} lands in shared memory as a 128B-swizzled K-stack of 8-row
-// atoms, exactly the canonical MN-major SWIZZLE_128B layout a UMMA shared-memory descriptor describes.
-// ci4 spans are widened on chip (S1): nibble n -> byte n<<4 (= 16 n as int8), G comes out scaled by
-// 256 and every G entry is shifted back (exactly) in the epilogue.
+// z is "MN-major" for both MMA operands (the time axis is K): a TMA box {128 bytes of m, 1 channel, KT samples}
+// lands in shared memory as a 128B-swizzled K-stack of 8-row atoms, exactly the canonical MN-major SWIZZLE_128B
+// layout a UMMA shared-memory descriptor describes.
 //
-// Steps:  S1 unpack/transpose = TMA (+ unpack warps for ci4);
-// S2 = static lower-triangle tile table walked by persistent CTAs;  S3 = tcgen05.mma kind::i8, int32
-// accumulators resident in TMEM for the whole span;  S4 = TMEM -> registers -> 2x2 combine (lane-pair
-// shuffles) -> shared staging -> coalesced (read-modify-)write of the packed triangle.
-//
-// One CTA = 8 warps (+4 unpack warps for ci4):
-//   warp 0      TMA producer (one lane)
-//   warp 1      MMA issuer   (one lane)
-//   warp 2      TMEM allocator
-//   warps 4..7  epilogue, warp w owns TMEM lanes 32(w-4).. = real rows = 16 inputs of the tile
-//   warps 8..11 (ci4 only) raw nibble bytes -> swizzled int8 operand tiles
+// Steps:  S1 unpack-and-transpose = relayout warps -> L2-resident ring -> TMA (pair kernel),
+// or TMA -> unpack warps (few-input kernel);  S2 = dynamic hand-out of lower-triangle tiles;  S3 = tcgen05.mma
+// kind::i8, int32 accumulators resident in TMEM for the whole span;  S4 = TMEM -> registers -> 2x2 combine
+// (lane-pair shuffles) -> shared staging -> bulk store / L2 reduce-add into the packed triangle.
 #pragma once
 #include <cstdint>
 #include <cuda.h>
@@ -32,8 +24,6 @@
 namespace bfx {
 
 // ---- tile geometry ----------------------------------------------------------------------------
-constexpr int TC_BM_IN = 64;    // inputs per A tile  -> UMMA M = 128 real rows
-constexpr int TC_BN_IN = 128;   // inputs per B tile  -> UMMA N = 256 real columns (two 64-input boxes)
 // L2 eviction hints (A/B measured, profiles/round1.md): ring slabs evict_last, span reads and visibility writes evict_first
 #ifndef BFX_NO_L2_HINTS
 #define BFX_L2_HINTS 1
@@ -43,9 +33,6 @@ constexpr int TC_BN_IN = 128;   // inputs per B tile  -> UMMA N = 256 real colum
 #endif
 constexpr int TC_KT = BFX_KT;   // samples per pipeline stage (TC_KT / 32 MMAs of K = 32); one TMA box = TC_KT rows
 constexpr int TC_BOX_BYTES = TC_KT * 128;        // one operand box: KT rows of 128 bytes
-constexpr int TC_STAGE_BYTES = 3 * TC_BOX_BYTES; // A, B0, B1
-constexpr int TC_RAW_BOX_BYTES = TC_KT * 64;     // ci4: one raw box, KT rows of 64 bytes
-constexpr int TC_RAW_STAGE_BYTES = 3 * TC_RAW_BOX_BYTES;
 constexpr int TC_CJ = 64;                        // visibilities (columns j) per epilogue chunk
 constexpr int TC_STG_PITCH = TC_CJ * 8 + 8;      // staging row pitch: 130 words -> 16 rows hit 16 distinct bank pairs
 constexpr int TC_STG_BUF_BYTES = 16 * TC_STG_PITCH;   // one warp's 16 rows x 64 visibilities
@@ -53,38 +40,18 @@ constexpr int TC_STG_WARP_BYTES = 2 * TC_STG_BUF_BYTES;  // double buffered agai
 constexpr int TC_STG_BYTES = 4 * TC_STG_WARP_BYTES;
 constexpr int TC_TMEM_COLS = 512;                // two 256-column accumulators
 
-template <bool CI4>
-struct TcCfg {
-    static constexpr int kOpStages = (CI4 ? 4 : 6) * 64 / TC_KT;   // int8 operand ring the MMA reads
-    static constexpr int kRawStages = CI4 ? 4 * 64 / TC_KT : 0;  // ci4: raw byte ring the TMA fills
-    static constexpr int kThreads = CI4 ? 384 : 512;  // direct ci4: 4 unpack warps; else up to 8 relayout warps
-    static constexpr int kSmemBytes = 1024 /*align slack*/ + kOpStages * TC_STAGE_BYTES +
-                                      kRawStages * TC_RAW_STAGE_BYTES + TC_STG_BYTES + 512 /*barriers*/;
-};
-
-// One entry of the lower-triangle tile table (S2), built on the host by bfXcorrCreate.
-struct TcTile {
-    int16_t row_blk;   // r: inputs [64 r, 64 r + 64)
-    int16_t col_blk;   // cb: inputs [128 cb, 128 cb + 128)
-    int8_t nbox;       // 1 -> UMMA N = 128, 2 -> UMMA N = 256
-    int8_t a_alias;    // -1: A has its own box; 0/1: A is B's box 0/1 (diagonal tiles: A block == B block)
-    int16_t pad;
-};
-
 struct TcParams {
     int32_t* out;
-    const TcTile* tiles;     // 1-CTA kernel: 64 x 128-input tiles
-    const void* pair_tiles;  // CTA-pair kernel: 128 x 128-input tiles (PrTile)
     int ninputs, nchan, ntime;
     int tiles_per_chan;
     long long ntiles;  // tiles_per_chan * nchan
     int accumulate;
     unsigned long long* sched;  // [0] next tile to hand out, [1] CTAs finished (self-resetting, see tc_next_tile)
-    // ---- S1 fused into this kernel (rl_enabled): the operands are read from a ring `z` of ring_w channel
+    // ---- S1 fused into the pair kernel: the operands are read from a ring `z` of ring_w channel
     // slabs, z[c % ring_w][t][2 i + part] int8, that the relayout warps fill from the span `x`
     // ahead of the tiles being contracted.  ready[c] / done[c] count, over all launches of the
     // plan, the relayout units written for channel c / the tiles of channel c whose loads have landed.
-    int rl_enabled, rl_ci4;
+    int rl_ci4;
     const uint8_t* x;
     uint8_t* z;
     int row_in;             // bytes of one (t, c) row of the span
@@ -383,253 +350,6 @@ __device__ __forceinline__ void tc_relayout_role(const TcParams& p, uint32_t lan
         u = __shfl_sync(0xffffffffu, u, 0);
         if (u >= total_units) break;
         do_unit(static_cast<int>(u / p.rl_units), static_cast<int>(u % p.rl_units));
-    }
-}
-
-template <bool CI4>
-__global__ void __launch_bounds__(TcCfg<CI4>::kThreads, 1)
-xcorr_tcgen05_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
-{
-    using Cfg = TcCfg<CI4>;
-    constexpr int S = Cfg::kOpStages;
-    constexpr int R = CI4 ? Cfg::kRawStages : 1;
-
-    extern __shared__ uint8_t smem_raw[];
-    const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
-    const uint32_t op_base = smem_base;                                    // S stages of (A, B0, B1) int8 operands
-    const uint32_t raw_base = op_base + S * TC_STAGE_BYTES;                // ci4: raw nibble-byte ring
-    const uint32_t stg_base = raw_base + Cfg::kRawStages * TC_RAW_STAGE_BYTES;
-    const uint32_t bar_base = stg_base + TC_STG_BYTES;
-    // barriers (8 bytes each)
-    const uint32_t bar_full = bar_base;                // [S]  operands ready for the MMA
-    const uint32_t bar_empty = bar_full + 8 * S;       // [S]  MMAs that read the stage have completed
-    const uint32_t bar_tfull = bar_empty + 8 * S;      // [2]  accumulator complete
-    const uint32_t bar_tempty = bar_tfull + 16;        // [2]  accumulator drained by the epilogue
-    const uint32_t bar_rfull = bar_tempty + 16;        // [R]  ci4: raw bytes landed
-    const uint32_t bar_rempty = bar_rfull + 8 * R;     // [R]  ci4: raw bytes consumed
-    const uint32_t tmem_slot = bar_rempty + 8 * R;     // 4 bytes: TMEM base address (8 reserved)
-    const uint32_t bar_sfull = tmem_slot + 8;          // [TC_RING] scheduled tile index published
-    const uint32_t bar_sempty = bar_sfull + 8 * TC_RING;  // [TC_RING] every consumer role has read it
-    const uint32_t ring_base = bar_sempty + 8 * TC_RING;  // [TC_RING] int64 tile index, -1 = no more work
-
-    const int warp = threadIdx.x >> 5;
-    const uint32_t lane = ptx::lane_id();
-
-    if (warp == 0 && lane == 0) {
-        ptx::prefetch_tensormap(&tmap);
-        for (int s = 0; s < S; ++s) {
-            ptx::mbar_init(bar_full + 8 * s, CI4 ? 4 : 1);
-            ptx::mbar_init(bar_empty + 8 * s, 1);
-        }
-        for (int b = 0; b < 2; ++b) {
-            ptx::mbar_init(bar_tfull + 8 * b, 1);
-            ptx::mbar_init(bar_tempty + 8 * b, 4);
-        }
-        if (CI4)
-            for (int s = 0; s < R; ++s) {
-                ptx::mbar_init(bar_rfull + 8 * s, 1);
-                ptx::mbar_init(bar_rempty + 8 * s, 4);
-            }
-        for (int s = 0; s < TC_RING; ++s) {
-            ptx::mbar_init(bar_sfull + 8 * s, 1);
-            // MMA issuer + 4 epilogue warps (+ 4 unpack warps)
-            ptx::mbar_init(bar_sempty + 8 * s, CI4 ? 9 : 5);
-        }
-        ptx::fence_barrier_init();
-    }
-    if (warp == 2) {
-        ptx::tmem_alloc<1>(tmem_slot, TC_TMEM_COLS);
-        ptx::tmem_relinquish<1>();
-    }
-    ptx::tc_fence_before();
-    __syncthreads();
-    ptx::tc_fence_after();
-    uint32_t tmem_base;
-    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
-
-    const int nkb = (p.ntime + TC_KT - 1) / TC_KT;
-    const TcRing ring{bar_sfull, bar_sempty, ring_base};
-
-    if (warp == 0) {
-        // ===================== TMA producer (S1 for ci8, first half of S1 for ci4) =====================
-        if (lane == 0) {
-            uint32_t stage = 0, phase = 0;
-            int ready_chan = -1;
-            constexpr int NST = CI4 ? R : S;
-            for (uint32_t n = 0;; ++n) {
-                ring.wait_free(n);
-                long long w = static_cast<long long>(atomicAdd(p.sched, 1ull));
-                if (w >= p.ntiles) w = -1;
-                ring.publish(n, w);
-                if (w < 0) break;
-                const int c = static_cast<int>(w / p.tiles_per_chan);
-                const int q = static_cast<int>(w % p.tiles_per_chan);
-                const TcTile tl = p.tiles[q];
-                if (!CI4 && p.rl_enabled && c != ready_chan) {
-                    // the relayout warps (of any CTA) must have
-                    // written all of z[c]; their generic-proxy stores are then ordered before our TMA (async proxy) reads
-                    const unsigned long long want = p.epoch * static_cast<unsigned long long>(p.rl_units);
-                    uint32_t spins = 0;
-                    while (ptx::ld_acquire_u64(p.ready + c) < want)
-                        if (++spins > (1u << 26)) __trap();
-                    ptx::fence_proxy_async_global();
-                    ready_chan = c;
-                }
-                const int xbytes = CI4 ? 64 : 128;  // bytes of one 64-input block in a span row
-                const int xa = tl.row_blk * xbytes;
-                const int xb = tl.col_blk * 2 * xbytes;
-                const uint32_t box = CI4 ? TC_RAW_BOX_BYTES : TC_BOX_BYTES;
-                const uint32_t nbytes = box * (tl.nbox + (tl.a_alias < 0 ? 1 : 0));
-                const int cs = (!CI4 && p.rl_enabled) ? c % p.ring_w : c;  // channel coordinate in the operand source
-                for (int kb = 0; kb < nkb; ++kb) {
-                    const uint32_t fullb = (CI4 ? bar_rfull : bar_full) + 8 * stage;
-                    const uint32_t emptyb = (CI4 ? bar_rempty : bar_empty) + 8 * stage;
-                    ptx::mbar_wait(emptyb, phase ^ 1);
-                    ptx::mbar_expect_tx(fullb, nbytes);
-                    const uint32_t dst = CI4 ? raw_base + stage * TC_RAW_STAGE_BYTES : op_base + stage * TC_STAGE_BYTES;
-                    const int t0 = kb * TC_KT;
-                    if (tl.a_alias < 0) ptx::tma_load_3d(dst, &tmap, fullb, xa, cs, t0);
-                    ptx::tma_load_3d(dst + box, &tmap, fullb, xb, cs, t0);
-                    if (tl.nbox > 1) ptx::tma_load_3d(dst + 2 * box, &tmap, fullb, xb + xbytes, cs, t0);
-                    if (++stage == NST) { stage = 0; phase ^= 1; }
-                }
-            }
-        }
-    } else if (warp == 1) {
-        // ===================== MMA issuer (S3) =====================
-        if (lane == 0) {
-            uint32_t stage = 0, phase = 0;
-            for (uint32_t it = 0;; ++it) {
-                const long long w = ring.get<false>(it, 0);
-                if (w < 0) break;
-                const TcTile tl = p.tiles[w % p.tiles_per_chan];
-                const uint32_t buf = it & 1, bphase = (it >> 1) & 1;
-                const uint32_t idesc = tc_instr_desc(128, 128 * tl.nbox);
-                const uint32_t d_tmem = tmem_base + buf * 256;
-                ptx::mbar_wait(bar_tempty + 8 * buf, bphase ^ 1);
-                ptx::tc_fence_after();
-                for (int kb = 0; kb < nkb; ++kb) {
-                    ptx::mbar_wait(bar_full + 8 * stage, phase);
-                    ptx::tc_fence_after();
-                    const uint32_t sbase = op_base + stage * TC_STAGE_BYTES;
-                    const uint32_t a_addr = sbase + (tl.a_alias < 0 ? 0 : (1 + tl.a_alias) * TC_BOX_BYTES);
-                    const uint64_t adesc = tc_smem_desc(a_addr, TC_BOX_BYTES);
-                    const uint64_t bdesc = tc_smem_desc(sbase + TC_BOX_BYTES, TC_BOX_BYTES);
-                    const int trem = p.ntime - kb * TC_KT;
-                    const int nk = trem >= TC_KT ? TC_KT / 32 : (trem + 31) / 32;
-                    for (int k = 0; k < nk; ++k) {
-                        // advance 32 K rows = 32 * 128 B -> +256 in the (addr >> 4) field
-                        ptx::mma_i8<1>(d_tmem, adesc + 256u * k, bdesc + 256u * k, idesc, (kb | k) != 0 ? 1u : 0u);
-                    }
-                    ptx::mma_commit(bar_empty + 8 * stage);
-                    if (++stage == S) { stage = 0; phase ^= 1; }
-                }
-                ptx::mma_commit(bar_tfull + 8 * buf);
-                // every operand load of this tile has landed in shared memory (observed through the full barriers, so a
-                // relaxed count is enough): its ring slab may be recycled
-                if (!CI4 && p.rl_enabled) ptx::red_relaxed_add_u64(p.done + w / p.tiles_per_chan, 1ull);
-            }
-        }
-    } else if (warp >= 4 && warp < 8) {
-        // ===================== epilogue (S4) =====================
-        const int wq = warp - 4;                      // TMEM lane quarter
-        const uint32_t stg_warp = stg_base + wq * TC_STG_WARP_BYTES;
-        const long long nbl = static_cast<long long>(p.ninputs) * (p.ninputs + 1) / 2;
-        uint32_t nchunks_done = 0;
-        for (uint32_t it = 0;; ++it) {
-            const long long w = ring.get<true>(it, lane);
-            if (w < 0) break;
-            const int c = static_cast<int>(w / p.tiles_per_chan);
-            const TcTile tl = p.tiles[w % p.tiles_per_chan];
-            const uint32_t buf = it & 1, bphase = (it >> 1) & 1;
-            const int i0 = tl.row_blk * TC_BM_IN + 16 * wq;  // first input row this warp owns
-            const int j0 = tl.col_blk * TC_BN_IN;
-            const int nchunk = tl.nbox;                       // 64 visibilities columns per chunk
-            int32_t* const out_c = p.out + 2 * (static_cast<long long>(c) * nbl);
-
-            ptx::mbar_wait(bar_tfull + 8 * buf, bphase);
-            ptx::tc_fence_after();
-            for (int jc = 0; jc < nchunk; ++jc, ++nchunks_done) {
-                const uint32_t stg_buf = stg_warp + (nchunks_done & 1) * TC_STG_BUF_BYTES;
-                const uint32_t tcol = tmem_base + (static_cast<uint32_t>(32 * wq) << 16) + buf * 256 + jc * 128;
-                tc_epilogue_chunk<CI4>(p, lane, tcol, stg_buf, out_c, i0, j0 + jc * TC_CJ,
-                                       jc == nchunk - 1 ? bar_tempty + 8 * buf : 0u);
-            }
-        }
-        if (lane < 16) ptx::bulk_wait_read<0>();  // shared memory must outlive the bulk reads
-    } else if (CI4 && warp >= 8) {
-        // ===================== ci4 unpack warps (second half of S1) =====================
-        // raw stage: 3 boxes [KT][64 B] (one byte per sample: re<<4 | im&15, include/bfxcorr.h)
-        // operand stage: 3 boxes [KT][128 B], byte 2i = re_i << 4, byte 2i+1 = im_i << 4, 16-byte chunks
-        // XOR-swizzled by (t & 7) exactly as TMA SWIZZLE_128B would have written them.
-        const int uw = warp - 8;
-        const int tid = uw * 32 + static_cast<int>(lane);  // 0..127
-        uint32_t rstage = 0, rphase = 0, ostage = 0, ophase = 0;
-        for (uint32_t it = 0;; ++it) {
-            const long long w = ring.get<true>(it, lane);
-            if (w < 0) break;
-            const TcTile tl = p.tiles[w % p.tiles_per_chan];
-            const int first_box = tl.a_alias < 0 ? 0 : 1;
-            const int last_box = tl.nbox;  // boxes first_box..last_box inclusive
-            for (int kb = 0; kb < nkb; ++kb) {
-                ptx::mbar_wait(bar_rfull + 8 * rstage, rphase);
-                ptx::mbar_wait(bar_empty + 8 * ostage, ophase ^ 1);
-                const uint32_t rsrc = raw_base + rstage * TC_RAW_STAGE_BYTES;
-                const uint32_t odst = op_base + ostage * TC_STAGE_BYTES;
-                for (int bx = first_box; bx <= last_box; ++bx) {
-                    // KT rows x 4 chunks of 16 bytes = 256 chunk-tasks per box, 2 per thread
-#pragma unroll
-                    for (int e = 0; e < (TC_KT * 4) / 128; ++e) {
-                        const int task = tid + 128 * e;
-                        const int t = task >> 2, qc = task & 3;
-                        uint32_t wv[4];
-                        const uint32_t ra = rsrc + bx * TC_RAW_BOX_BYTES + t * 64 + qc * 16;
-                        asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
-                                     : "=r"(wv[0]), "=r"(wv[1]), "=r"(wv[2]), "=r"(wv[3])
-                                     : "r"(ra));
-                        uint32_t o[8];
-#pragma unroll
-                        for (int u = 0; u < 4; ++u) {
-                            const uint32_t hi = wv[u] & 0xF0F0F0F0u;          // 4 x (re << 4)
-                            const uint32_t lo = (wv[u] << 4) & 0xF0F0F0F0u;   // 4 x (im << 4)
-                            o[2 * u] = __byte_perm(hi, lo, 0x5140);           // re0 im0 re1 im1
-                            o[2 * u + 1] = __byte_perm(hi, lo, 0x7362);       // re2 im2 re3 im3
-                        }
-                        const uint32_t rowa = odst + bx * TC_BOX_BYTES + t * 128;
-                        const uint32_t c0 = static_cast<uint32_t>((2 * qc) ^ (t & 7)) * 16;
-                        const uint32_t c1 = static_cast<uint32_t>((2 * qc + 1) ^ (t & 7)) * 16;
-                        asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(rowa + c0), "r"(o[0]), "r"(o[1]),
-                                     "r"(o[2]), "r"(o[3])
-                                     : "memory");
-                        asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(rowa + c1), "r"(o[4]), "r"(o[5]),
-                                     "r"(o[6]), "r"(o[7])
-                                     : "memory");
-                    }
-                }
-                ptx::fence_proxy_async_smem();  // generic-proxy stores -> visible to the tensor core (async proxy)
-                __syncwarp();
-                if (lane == 0) {
-                    ptx::mbar_arrive(bar_rempty + 8 * rstage);
-                    ptx::mbar_arrive(bar_full + 8 * ostage);
-                }
-                if (++rstage == R) { rstage = 0; rphase ^= 1; }
-                if (++ostage == S) { ostage = 0; ophase ^= 1; }
-            }
-        }
-    }
-
-    else if (!CI4 && warp >= 8 && p.rl_enabled) {
-        tc_relayout_role(p, lane);
-    }
-
-    ptx::tc_fence_before();
-    __syncthreads();
-    if (warp == 2) ptx::tmem_dealloc<1>(tmem_base, TC_TMEM_COLS);
-    // the last CTA to finish re-arms the scheduler for the next launch (every CTA has drawn its final index)
-    if (threadIdx.x == 0 && atomicAdd(p.sched + 1, 1ull) == gridDim.x - 1) {
-        p.sched[0] = 0;
-        p.sched[1] = 0;
-        p.sched[2] = 0;
     }
 }
 

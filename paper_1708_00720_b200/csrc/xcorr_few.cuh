@@ -1,34 +1,42 @@
-// xcorr_few.cuh -- few-input ci4 spans (ninputs <= 64: one 64 x 64-input tile per channel), the bandwidth-bound
-// case of BASELINE.json configs[4].  Every sample is used by exactly one tile, so there is no re-read to save and
-// the span is consumed in place; what limits a per-channel kernel is address translation: a channel's samples
-// are 64-byte pieces lying nchan*64 bytes (1 MiB on cfg5) apart, two per 2 MiB page, and the TMA unit delivered
-// 6.5 B/clk/SM on them (profiles/round1.md).  Here one CTA contracts FW_NC = 4 ADJACENT channels at once, so each
-// TMA box row is a contiguous run of 4 x 64 bytes and the translations per byte drop fourfold; the four
+// xcorr_few.cuh -- few-input spans (ninputs <= 64: one 64 x 64-input tile per channel), the bandwidth-bound case
+// of BASELINE.json configs[4].  Every sample is used by exactly one tile, so there is no re-read to save and the
+// span is consumed in place; what limits a per-channel kernel is address translation and DRAM locality: a
+// channel's samples are 64..128-byte pieces lying nchan*row bytes (1 MiB on cfg5) apart, and the TMA unit
+// delivered 6.5 B/clk/SM on them (profiles/round1.md).  Here one CTA contracts FW_NC = 4 ADJACENT channels at
+// once, so each TMA box row is a contiguous run of 4 rows and the translations per byte drop fourfold; the four
 // 128-lane x 128-column accumulators fill the CTA's 512 TMEM columns.
 //
-// Roles (512 threads): warp 0 TMA producer (raw nibble bytes, box {row bytes, 4 channels, FW_KT samples}),
-// warp 1 MMA issuer (per channel: A = B = the channel's int8 tile, M = 128, N = 128), warp 2 TMEM allocator,
-// warps 4..7 epilogue (tc_epilogue_chunk, one 64-visibility chunk per channel), warps 8..15 unpack: raw bytes ->
-// 128B-swizzled int8 tiles (nibble << 4; the 16 x 16 scale is shifted out exactly in the epilogue).
+// Roles (512 threads): warp 0 TMA producer (raw bytes, box {row bytes, 4 channels, FW_KT samples}), warp 1 MMA
+// issuer (per channel: A = B = the channel's int8 tile, M = 128, N = 128), warp 2 TMEM allocator, warps 4..7
+// epilogue (tc_epilogue_chunk, one 64-visibility chunk per channel), warps 8..15 unpack: raw [t][c][row] bytes ->
+// per-channel 128B-swizzled int8 tiles (ci4: nibble << 4, the 16 x 16 scale is shifted out exactly in the
+// epilogue; ci8: a swizzling copy).
 #pragma once
-#include "xcorr_tcgen05.cuh"
+#include "xcorr_common.cuh"
 
 namespace bfx {
 
 constexpr int FW_NC = 4;     // channels per CTA tile
 constexpr int FW_KT = 64;    // samples per stage
-constexpr int FW_RAW_STAGES = 3, FW_OP_STAGES = 3;
-constexpr int FW_RAW_STAGE_BYTES = FW_KT * FW_NC * 64;    // [t][c][<= 64 B]
 constexpr int FW_OP_TILE_BYTES = FW_KT * 128;             // one channel: [t][128 B] swizzled
 constexpr int FW_OP_STAGE_BYTES = FW_NC * FW_OP_TILE_BYTES;
 constexpr int FW_UNPACK_WARPS = 8;
 constexpr int FW_THREADS = 256 + 32 * FW_UNPACK_WARPS;
-constexpr int FW_SMEM_BYTES = 1024 + FW_RAW_STAGES * FW_RAW_STAGE_BYTES + FW_OP_STAGES * FW_OP_STAGE_BYTES + TC_STG_BYTES + 512;
 
+template <bool CI4>
+struct FwCfg {
+    static constexpr int kRawRow = CI4 ? 64 : 128;                     // bytes of a 64-input raw row
+    static constexpr int kRawStageBytes = FW_KT * FW_NC * kRawRow;     // [t][c][<= kRawRow]
+    static constexpr int kRawStages = CI4 ? 3 : 2, kOpStages = CI4 ? 3 : 2;
+    static constexpr int kSmemBytes = 1024 + kRawStages * kRawStageBytes + kOpStages * FW_OP_STAGE_BYTES + TC_STG_BYTES + 512;
+};
+
+template <bool CI4>
 __global__ void __launch_bounds__(FW_THREADS, 1)
 xcorr_few_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
 {
-    constexpr int R = FW_RAW_STAGES, S = FW_OP_STAGES;
+    constexpr int R = FwCfg<CI4>::kRawStages, S = FwCfg<CI4>::kOpStages;
+    constexpr int FW_RAW_STAGE_BYTES = FwCfg<CI4>::kRawStageBytes;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
     const uint32_t op_base = smem_base;
@@ -48,7 +56,7 @@ xcorr_few_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
 
     const int warp = threadIdx.x >> 5;
     const uint32_t lane = ptx::lane_id();
-    const int row = p.row_in;  // ninputs bytes per (t, c), a multiple of 16, <= 64
+    const int row = p.row_in;  // bytes per (t, c): ninputs (ci4) or 2 * ninputs (ci8), a multiple of 16
 
     // the int8 tiles are 128 bytes wide; with fewer than 64 inputs the unpack warps never touch the right part
     for (uint32_t o = threadIdx.x * 16; o < S * FW_OP_STAGE_BYTES; o += FW_THREADS * 16)
@@ -165,7 +173,7 @@ xcorr_few_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
                 const uint32_t stg_buf = stg_warp + (nchunks_done & 1) * TC_STG_BUF_BYTES;
                 const uint32_t tcol = tmem_base + (static_cast<uint32_t>(32 * wq) << 16) + 128 * ch;
                 int32_t* const out_c = p.out + 2 * (static_cast<long long>(c0 + ch) * nbl);
-                tc_epilogue_chunk<true, false>(p, lane, tcol, stg_buf, out_c, 16 * wq, 0, ch == nch - 1 ? bar_tempty : 0u);
+                tc_epilogue_chunk<CI4, false>(p, lane, tcol, stg_buf, out_c, 16 * wq, 0, ch == nch - 1 ? bar_tempty : 0u);
             }
             if (nch == 0) {
                 ptx::tc_fence_before();
@@ -176,10 +184,15 @@ xcorr_few_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
         if (lane < 16) ptx::bulk_wait_read<0>();  // shared memory must outlive the bulk reads
     } else if (warp >= 8) {
         // ===================== unpack warps (S1): raw [t][c][row] nibble bytes -> per-channel int8 tiles =====================
-        // int8 tile: [t][128 B], byte 2i = re_i << 4, byte 2i+1 = im_i << 4, 16-byte chunks XOR-swizzled by (t & 7)
-        // exactly as TMA SWIZZLE_128B would have written them.
-        const int uw = warp - 8, tl = static_cast<int>(lane >> 2), qc = static_cast<int>(lane & 3);
-        const int qn = row >> 4;                                    // 16-byte chunks per raw row (1..4)
+        // int8 tile: [t][128 B], byte 2i = re_i (ci4: << 4), byte 2i+1 = im_i (ci4: << 4), 16-byte chunks XOR-swizzled
+        // by (t & 7) exactly as TMA SWIZZLE_128B would have written them.
+        // lane -> (row t, 16-byte chunk qc) of one channel; a quarter-warp writes whole swizzled rows, which touches
+        // every bank once; no divisions on the way.  ci4: 4 chunks of 16 samples per row, each widened to two int8
+        // chunks; ci8: 8 chunks per row, copied to their swizzled place.
+        constexpr int QPR = CI4 ? 4 : 8;   // raw chunks per full row
+        constexpr int RPW = 32 / QPR;      // rows per warp pass
+        const int uw = warp - 8, tl = static_cast<int>(lane) / QPR, qc = static_cast<int>(lane) % QPR;
+        const int qn = row >> 4;           // 16-byte chunks this span's rows really have
         uint32_t rstage = 0, rphase = 0, ostage = 0, ophase = 0;
         for (uint32_t it = 0;; ++it) {
             const long long w = ring.get<true>(it, lane);
@@ -189,30 +202,33 @@ xcorr_few_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
                 ptx::mbar_wait(bar_empty + 8 * ostage, ophase ^ 1);
                 const uint32_t rsrc = raw_base + rstage * FW_RAW_STAGE_BYTES;
                 const uint32_t odst = op_base + ostage * FW_OP_STAGE_BYTES;
-                // lane -> (row t, 16-byte chunk qc) of one channel: a quarter-warp writes 2 rows x 4 chunks of a
-                // swizzled tile, which touches every bank once; no divisions on the way
 #pragma unroll
                 for (int ch = 0; ch < FW_NC; ++ch) {
 #pragma unroll
-                    for (int t = uw * 8 + tl; t < FW_KT; t += 8 * FW_UNPACK_WARPS) {
+                    for (int t = uw * RPW + tl; t < FW_KT; t += RPW * FW_UNPACK_WARPS) {
                         if (qc < qn) {
                             uint32_t wv[4];
                             asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
                                          : "=r"(wv[0]), "=r"(wv[1]), "=r"(wv[2]), "=r"(wv[3])
                                          : "r"(rsrc + (t * FW_NC + ch) * row + qc * 16));
-                            uint32_t o[8];
-#pragma unroll
-                            for (int u = 0; u < 4; ++u) {
-                                const uint32_t hi = wv[u] & 0xF0F0F0F0u;          // 4 x (re << 4)
-                                const uint32_t lo = (wv[u] << 4) & 0xF0F0F0F0u;   // 4 x (im << 4)
-                                o[2 * u] = __byte_perm(hi, lo, 0x5140);           // re0 im0 re1 im1
-                                o[2 * u + 1] = __byte_perm(hi, lo, 0x7362);       // re2 im2 re3 im3
-                            }
                             const uint32_t rowa = odst + ch * FW_OP_TILE_BYTES + t * 128;
-                            const uint32_t a0 = rowa + static_cast<uint32_t>((2 * qc) ^ (t & 7)) * 16;
-                            const uint32_t a1 = rowa + static_cast<uint32_t>((2 * qc + 1) ^ (t & 7)) * 16;
-                            asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(a0), "r"(o[0]), "r"(o[1]), "r"(o[2]), "r"(o[3]) : "memory");
-                            asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(a1), "r"(o[4]), "r"(o[5]), "r"(o[6]), "r"(o[7]) : "memory");
+                            if (CI4) {
+                                uint32_t o[8];
+#pragma unroll
+                                for (int u = 0; u < 4; ++u) {
+                                    const uint32_t hi = wv[u] & 0xF0F0F0F0u;          // 4 x (re << 4)
+                                    const uint32_t lo = (wv[u] << 4) & 0xF0F0F0F0u;   // 4 x (im << 4)
+                                    o[2 * u] = __byte_perm(hi, lo, 0x5140);           // re0 im0 re1 im1
+                                    o[2 * u + 1] = __byte_perm(hi, lo, 0x7362);       // re2 im2 re3 im3
+                                }
+                                const uint32_t a0 = rowa + static_cast<uint32_t>((2 * qc) ^ (t & 7)) * 16;
+                                const uint32_t a1 = rowa + static_cast<uint32_t>((2 * qc + 1) ^ (t & 7)) * 16;
+                                asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(a0), "r"(o[0]), "r"(o[1]), "r"(o[2]), "r"(o[3]) : "memory");
+                                asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(a1), "r"(o[4]), "r"(o[5]), "r"(o[6]), "r"(o[7]) : "memory");
+                            } else {
+                                const uint32_t a0 = rowa + static_cast<uint32_t>(qc ^ (t & 7)) * 16;
+                                asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(a0), "r"(wv[0]), "r"(wv[1]), "r"(wv[2]), "r"(wv[3]) : "memory");
+                            }
                         }
                     }
                 }

@@ -1,5 +1,5 @@
 // xcorr_pair.cuh -- the X-engine contraction on CTA pairs (tcgen05 cta_group::2), the product path for
-// ninputs > 64.  Same method as xcorr_tcgen05.cuh (real Gram embedding, accumulators in TMEM for the whole
+// ninputs > 64.  Same method as xcorr_common.cuh (real Gram embedding, accumulators in TMEM for the whole
 // span, S1 relayout warps feeding an L2-resident ring, S4 bulk store / L2 reduce-add epilogue); what changes
 // is the tile: two CTAs of a cluster share one 128-input x 128-input tile,
 //
@@ -17,7 +17,7 @@
 // counter and publishes it to both CTAs' rings), 1 MMA issuer (leader only), 2 TMEM allocator, 4..7 epilogue,
 // 8..15 relayout (tc_relayout_role).
 #pragma once
-#include "xcorr_tcgen05.cuh"
+#include "xcorr_common.cuh"
 
 namespace bfx {
 
@@ -26,11 +26,6 @@ constexpr int PR_STAGES = 8 * 64 / TC_KT;
 constexpr int PR_STAGE_BYTES = 2 * TC_BOX_BYTES;    // A-half, B-half
 constexpr int PR_THREADS = 512;
 constexpr int PR_SMEM_BYTES = 1024 + PR_STAGES * PR_STAGE_BYTES + TC_STG_BYTES + 512;
-
-struct PrTile {
-    int16_t row_blk;  // R:  rows    [128 R,  128 R  + 128)
-    int16_t col_blk;  // Cb: columns [128 Cb, 128 Cb + 128), Cb <= R
-};
 
 // S2 decode without touching memory: tile index w -> (channel c, row block R, column block Cb <= R), tiles of a
 // channel enumerated row-major over the lower triangle of 128-input blocks: q = R (R + 1) / 2 + Cb.

@@ -1,7 +1,7 @@
 // xcorr_simt.cuh -- plain CUDA-core X-engine kernel (BF_XCORR_ALGO_SIMT).
 //
 // Not the product path: an on-device cross-check of the tcgen05 kernel at sizes the CPU oracle cannot
-// reach in test time (include/bfxcorr.h, bfXcorrAlgo).  It shares nothing with xcorr_tcgen05.cuh: own
+// reach in test time (include/bfxcorr.h, bfXcorrAlgo).  It shares nothing with the tensor-core kernels: own
 // decode, own tiling, own triangle indexing.
 //
 // One CTA = one channel x one 32x32 block of input pairs (I-block >= J-block); 256 threads, each
