@@ -107,11 +107,16 @@ int bfXcorrGetLaunchCount(bfXcorr plan, int* nlaunch);
 /* cudaError_t of the last failing CUDA call made on behalf of this plan (0 if none). */
 int bfXcorrGetLastCudaError(bfXcorr plan, int* cuda_error);
 
-/* Convenience for callers whose buffers live in HOST memory (bench.py's end-to-end leg): copies the
- * span host->device into plan-owned staging, executes, and -- if `out_host` is not NULL -- copies the
- * visibility buffer device->host, all on `stream`; `out_dev` is the persistent device accumulator.
- *   in_host, out_host : HOST pointers (pinned memory makes the copies asynchronous).
- *   errors            : as bfXcorrExecute, plus MEM_ALLOC_FAILED for the staging buffer. */
+/* Entry point for callers whose buffers live in HOST memory (bench.py's end-to-end leg).  The span is copied
+ * host->device into one of two plan-owned staging buffers on a private copy stream, the contraction runs on
+ * `stream` once the copy has landed, and -- if `out_host` is not NULL -- the visibility buffer is copied
+ * device->host on a second private stream that `stream` then waits for.  Successive calls therefore overlap the
+ * upload of span n+1 with the contraction of span n and with the download of the visibilities, as the paper's
+ * pipelines overlap copy and compute; synchronising `stream` still covers everything enqueued.
+ *   in_host, out_host : HOST pointers (pinned memory makes the copies asynchronous); `in_host` may be reused and
+ *                       `out_host` read once `stream` has been synchronised.
+ *   out_dev           : the persistent device accumulator, as in bfXcorrExecute.
+ *   errors            : as bfXcorrExecute, plus MEM_ALLOC_FAILED for the staging buffers. */
 int bfXcorrExecuteHost(bfXcorr plan, const void* in_host, void* out_dev, void* out_host, int accumulate,
                        void* stream);
 

@@ -45,8 +45,13 @@ struct bfXcorr_impl {
     int ring_w;
     unsigned long long* d_flags;  // ready[nchan], done[nchan]
     unsigned long long epoch;     // fused launches so far
-    // staging for bfXcorrExecuteHost
-    void* d_stage_in;
+    // bfXcorrExecuteHost: two device staging buffers for spans and private copy streams, so that the host->device
+    // copy of span n+1 overlaps the contraction of span n and the device->host copy of the visibilities
+    // (the GPU analogue of the paper's pipeline parallelism)
+    void* d_stage_in[2];
+    cudaStream_t s_h2d, s_d2h;
+    cudaEvent_t ev_h2d[2], ev_comp[2], ev_d2h;
+    unsigned long long host_calls;
 };
 
 namespace {
@@ -308,19 +313,40 @@ int bfXcorrExecuteHost(bfXcorr plan, const void* in_host, void* out_dev, void* o
     if (!valid(plan)) return BF_XCORR_INVALID_HANDLE;
     if (!in_host || !out_dev) return BF_XCORR_INVALID_POINTER;
     cudaStream_t s = static_cast<cudaStream_t>(stream);
-    cudaError_t e;
-    if (!plan->d_stage_in) {
-        e = cudaMalloc(&plan->d_stage_in, input_bytes(plan));
+    cudaError_t e = cudaSuccess;
+    if (!plan->s_h2d) {
+        e = cudaStreamCreateWithFlags(&plan->s_h2d, cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&plan->s_d2h, cudaStreamNonBlocking);
+        for (int b = 0; b < 2 && e == cudaSuccess; ++b) {
+            e = cudaMalloc(&plan->d_stage_in[b], input_bytes(plan));
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&plan->ev_h2d[b], cudaEventDisableTiming);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&plan->ev_comp[b], cudaEventDisableTiming);
+        }
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&plan->ev_d2h, cudaEventDisableTiming);
         if (e != cudaSuccess) return cuda_fail(plan, e);
     }
-    e = cudaMemcpyAsync(plan->d_stage_in, in_host, input_bytes(plan), cudaMemcpyHostToDevice, s);
+    const int b = static_cast<int>(plan->host_calls & 1);
+    // span -> staging[b] on the copy stream, once the contraction that last read staging[b] (two calls ago) is done
+    if (plan->host_calls >= 2) e = cudaStreamWaitEvent(plan->s_h2d, plan->ev_comp[b], 0);
+    if (e == cudaSuccess)
+        e = cudaMemcpyAsync(plan->d_stage_in[b], in_host, input_bytes(plan), cudaMemcpyHostToDevice, plan->s_h2d);
+    if (e == cudaSuccess) e = cudaEventRecord(plan->ev_h2d[b], plan->s_h2d);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(s, plan->ev_h2d[b], 0);
     if (e != cudaSuccess) return cuda_fail(plan, e);
-    const int st = bfXcorrExecute(plan, plan->d_stage_in, out_dev, accumulate, stream);
+    ++plan->host_calls;
+    const int st = bfXcorrExecute(plan, plan->d_stage_in[b], out_dev, accumulate, stream);
     if (st != BF_XCORR_OK) return st;
-    if (out_host) {
-        e = cudaMemcpyAsync(out_host, out_dev, output_bytes(plan), cudaMemcpyDeviceToHost, s);
-        if (e != cudaSuccess) return cuda_fail(plan, e);
+    e = cudaEventRecord(plan->ev_comp[b], s);
+    if (e == cudaSuccess && out_host) {
+        // visibilities -> host on the other copy stream; `stream` waits for it, so that synchronising `stream`
+        // covers the copy and no later launch touches out_dev while it is being read -- but the NEXT call's
+        // host->device copy runs on its own stream and overlaps this one (PCIe is full duplex)
+        e = cudaStreamWaitEvent(plan->s_d2h, plan->ev_comp[b], 0);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(out_host, out_dev, output_bytes(plan), cudaMemcpyDeviceToHost, plan->s_d2h);
+        if (e == cudaSuccess) e = cudaEventRecord(plan->ev_d2h, plan->s_d2h);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(s, plan->ev_d2h, 0);
     }
+    if (e != cudaSuccess) return cuda_fail(plan, e);
     return BF_XCORR_OK;
 }
 
@@ -328,7 +354,14 @@ int bfXcorrDestroy(bfXcorr plan)
 {
     if (!valid(plan)) return BF_XCORR_INVALID_HANDLE;
     if (plan->d_sched) cudaFree(plan->d_sched);
-    if (plan->d_stage_in) cudaFree(plan->d_stage_in);
+    for (int b = 0; b < 2; ++b) {
+        if (plan->d_stage_in[b]) cudaFree(plan->d_stage_in[b]);
+        if (plan->ev_h2d[b]) cudaEventDestroy(plan->ev_h2d[b]);
+        if (plan->ev_comp[b]) cudaEventDestroy(plan->ev_comp[b]);
+    }
+    if (plan->ev_d2h) cudaEventDestroy(plan->ev_d2h);
+    if (plan->s_h2d) cudaStreamDestroy(plan->s_h2d);
+    if (plan->s_d2h) cudaStreamDestroy(plan->s_d2h);
     if (plan->d_z) cudaFree(plan->d_z);
     if (plan->d_flags) cudaFree(plan->d_flags);
     plan->magic = 0;

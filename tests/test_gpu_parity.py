@@ -139,3 +139,40 @@ def test_tcgen05_equals_simt_mid_size(dtype):
     sub = [0, 11, 23]
     exp = oracle.xcorr(np.ascontiguousarray(x[:, sub]), N, len(sub), T, dtype)
     np.testing.assert_array_equal(a[sub], exp)
+
+
+@pytest.mark.parametrize("dtype", [4, 8])
+def test_execute_host_streams_spans(dtype):
+    """bfXcorrExecuteHost (include/bfxcorr.h): pinned host spans in, visibilities out, five spans through the two
+    staging buffers and the private copy streams; after synchronising the stream the host result is the oracle's."""
+    N, C, T = 192, 6, 150
+    rng = np.random.default_rng(31 + dtype)
+    xs = [rand_span(rng, T, C, N, dtype) for _ in range(5)]
+    exp = oracle.xcorr(xs[0], N, C, T, dtype)
+    for x in xs[1:]:
+        oracle.xcorr(x, N, C, T, dtype, out=exp, accumulate=True)
+    nb = N * (N + 1) // 2
+    dev = torch.device("cuda:0")
+    plan = bfx.bfXcorrCreate(N, C, T, dtype)
+    try:
+        out_dev = torch.full((C, nb, 2), 0x5A5A5A5A, dtype=torch.int32, device=dev)
+        out_host = torch.zeros((C, nb, 2), dtype=torch.int32).pin_memory()
+        hosts = [torch.from_numpy(np.ascontiguousarray(x)).reshape(-1).pin_memory() for x in xs]
+        stream = torch.cuda.current_stream().cuda_stream
+        for s, h in enumerate(hosts):
+            last = s == len(hosts) - 1
+            bfx.bfXcorrExecuteHost(plan, h.data_ptr(), out_dev.data_ptr(), out_host.data_ptr() if last else 0, s > 0, stream)
+        torch.cuda.synchronize()
+        np.testing.assert_array_equal(out_host.numpy(), exp)
+        np.testing.assert_array_equal(out_dev.cpu().numpy(), exp)
+        # a second round into the same plan, reusing one host buffer between calls (stream-synchronised)
+        for s in range(3):
+            hosts[0].copy_(torch.from_numpy(np.ascontiguousarray(xs[s])).reshape(-1))
+            bfx.bfXcorrExecuteHost(plan, hosts[0].data_ptr(), out_dev.data_ptr(), out_host.data_ptr(), s > 0, stream)
+            torch.cuda.synchronize()
+        exp3 = oracle.xcorr(xs[0], N, C, T, dtype)
+        for x in xs[1:3]:
+            oracle.xcorr(x, N, C, T, dtype, out=exp3, accumulate=True)
+        np.testing.assert_array_equal(out_host.numpy(), exp3)
+    finally:
+        bfx.bfXcorrDestroy(plan)
