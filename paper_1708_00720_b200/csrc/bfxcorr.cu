@@ -12,7 +12,6 @@
 #include "xcorr_simt.cuh"
 #include "xcorr_few.cuh"
 #include "xcorr_pair.cuh"
-#include "xcorr_quad.cuh"
 #include "xcorr_common.cuh"
 
 namespace {
@@ -160,41 +159,6 @@ int launch_tcgen05(bfXcorr p, const void* in, void* out, int accumulate, cudaStr
         prm.epoch = ++p->epoch;
     }
     cudaError_t e = cudaSuccess;
-#ifdef BFX_QUAD
-    if (pair) {
-        // clusters of four CTAs, two tiles per job (xcorr_quad.cuh)
-        const int nb = (p->ninputs + bfx::PR_BLK - 1) / bfx::PR_BLK;
-        int nshared = 0;
-        for (int r = 1; r < nb; ++r) nshared += (r + 1) / 2;
-        const int nleft = (nb + 1) / 2;
-        prm.qd_nb = nb;
-        prm.qd_nshared = nshared;
-        prm.qd_jobs_per_chan = nshared + (nleft + 1) / 2;
-        prm.ntiles = static_cast<long long>(prm.qd_jobs_per_chan) * p->nchan;
-        cudaLaunchConfig_t cfg;
-        std::memset(&cfg, 0, sizeof(cfg));
-        cfg.blockDim = dim3(bfx::PR_THREADS);
-        cfg.dynamicSmemBytes = bfx::PR_SMEM_BYTES;
-        cfg.stream = stream;
-        cudaLaunchAttribute attr;
-        attr.id = cudaLaunchAttributeClusterDimension;
-        attr.val.clusterDim.x = 4;
-        attr.val.clusterDim.y = 1;
-        attr.val.clusterDim.z = 1;
-        cfg.attrs = &attr;
-        cfg.numAttrs = 1;
-        cfg.gridDim = dim3(static_cast<unsigned>(p->num_sms / 4 * 4));
-        int nclusters = 0;
-        e = cudaOccupancyMaxActiveClusters(&nclusters, bfx::xcorr_quad_kernel, &cfg);
-        if (e == cudaSuccess) {
-            if (nclusters > p->num_sms / 4) nclusters = p->num_sms / 4;
-            if (nclusters > prm.ntiles) nclusters = static_cast<int>(prm.ntiles);
-            if (nclusters < 1) nclusters = 1;
-            cfg.gridDim = dim3(static_cast<unsigned>(4 * nclusters));
-            e = cudaLaunchKernelEx(&cfg, bfx::xcorr_quad_kernel, tmap, prm);
-        }
-    } else
-#endif
     if (pair) {
         // one cluster of two CTAs per tile in flight
         long long pairs = p->num_sms / 2;
@@ -317,8 +281,6 @@ int bfXcorrCreate(bfXcorr* plan, int ninputs, int nchan, int ntime, int dtype)
         e = cudaFuncSetAttribute(bfx::xcorr_few_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bfx::FwCfg<true>::kSmemBytes);
     if (e == cudaSuccess)
         e = cudaFuncSetAttribute(bfx::xcorr_few_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bfx::FwCfg<false>::kSmemBytes);
-    if (e == cudaSuccess)
-        e = cudaFuncSetAttribute(bfx::xcorr_quad_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bfx::PR_SMEM_BYTES);
     if (e == cudaSuccess)
         e = cudaFuncSetAttribute(bfx::xcorr_pair_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bfx::PR_SMEM_BYTES);
     if (e != cudaSuccess) {

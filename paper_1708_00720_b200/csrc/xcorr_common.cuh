@@ -61,8 +61,6 @@ struct TcParams {
     unsigned long long* ready;
     unsigned long long* done;
     unsigned long long epoch;  // 1, 2, ... : launch number of this plan
-    // xcorr_quad.cuh: jobs (two tiles) per channel, how many of them share a row block, 128-input blocks per edge
-    int qd_jobs_per_chan, qd_nshared, qd_nb;
 };
 
 #ifndef BFX_RL_ROWS
