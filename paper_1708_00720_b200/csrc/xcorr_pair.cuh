@@ -22,7 +22,10 @@
 namespace bfx {
 
 constexpr int PR_BLK = 128;                         // inputs per tile edge
-constexpr int PR_STAGES = 8 * 64 / TC_KT;
+#ifndef BFX_PR_STAGES
+#define BFX_PR_STAGES (8 * 64 / BFX_KT)
+#endif
+constexpr int PR_STAGES = BFX_PR_STAGES;
 constexpr int PR_STAGE_BYTES = 2 * TC_BOX_BYTES;    // A-half, B-half
 constexpr int PR_THREADS = 512;
 constexpr int PR_SMEM_BYTES = 1024 + PR_STAGES * PR_STAGE_BYTES + TC_STG_BYTES + 512;
