@@ -176,3 +176,25 @@ def test_execute_host_streams_spans(dtype):
         np.testing.assert_array_equal(out_host.numpy(), exp3)
     finally:
         bfx.bfXcorrDestroy(plan)
+
+
+def test_random_shapes_sweep():
+    """Seeded sweep over ragged shapes of both kernels (few-input: 4 channels per CTA with channel tails and rows of
+    16..128 bytes; pair kernel: partial 128-input blocks, odd tile counts), both dtypes, with and without accumulation."""
+    rng = np.random.default_rng(20240611)
+    for case in range(24):
+        dtype = 4 if case % 2 else 8
+        step = 16 if dtype == 4 else 8
+        if case % 3 == 0:
+            N = step * int(rng.integers(1, 64 // step + 1))          # few-input kernel
+        else:
+            N = step * int(rng.integers(64 // step + 1, 400 // step))  # pair kernel
+        C = int(rng.integers(1, 12))
+        T = int(rng.integers(1, 300))
+        nsp = int(rng.integers(1, 4))
+        xs = [rand_span(rng, T, C, N, dtype) for _ in range(nsp)]
+        exp = oracle.xcorr(xs[0], N, C, T, dtype)
+        for x in xs[1:]:
+            oracle.xcorr(x, N, C, T, dtype, out=exp, accumulate=True)
+        got = run_spans(xs, N, C, T, dtype, bfx.BF_XCORR_ALGO_TCGEN05)
+        np.testing.assert_array_equal(got, exp, err_msg="N=%d C=%d T=%d ci%d spans=%d" % (N, C, T, dtype, nsp))
