@@ -9,6 +9,7 @@ from .xcorr_oracle import (  # noqa: F401
     build,
     xcorr,
     xcorr_entries,
+    dump,
     threads,
     set_threads,
 )

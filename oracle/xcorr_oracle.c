@@ -150,6 +150,24 @@ long long xcorr_oracle(const uint8_t* in, int32_t* out, int ninputs, int nchan, 
 }
 
 /* Number of threads the span routine will use (1 when built without OpenMP). */
+/* Integration dump (the paper's accumulate block hands an integration on when it is
+ * complete, and its pipelines convert integer data to floating point for the stages that follow,
+ * PAPER.md:549): every int32 component v of the packed visibility buffer becomes the float32
+ *        f = (float) v * scale          (int32 -> float32 round-to-nearest-even, then one float32 multiply)
+ * in the same [nchan][B][2] order, and, if zero_acc != 0, the accumulator is cleared afterwards so that the next
+ * integration can start with accumulate = 1.  Returns the number of components converted, or -1 on bad arguments. */
+long long xcorr_oracle_dump(int32_t* acc, float* out, long long ncomponents, float scale, int zero_acc)
+{
+    long long k;
+    if (!acc || !out || ncomponents < 0) return -1;
+    for (k = 0; k < ncomponents; ++k) {
+        const float f = (float)acc[k];
+        out[k] = f * scale;
+        if (zero_acc) acc[k] = 0;
+    }
+    return ncomponents;
+}
+
 #ifdef _OPENMP
 #include <omp.h>
 int xcorr_oracle_threads(void) { return omp_get_max_threads(); }

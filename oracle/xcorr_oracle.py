@@ -113,6 +113,19 @@ def xcorr_entries(x: np.ndarray, ninputs: int, nchan: int, ntime: int, dtype: in
     return vals
 
 
+def dump(acc: np.ndarray, scale: float = 1.0, zero_acc: bool = False) -> np.ndarray:
+    """Integration dump: int32 [..][2] accumulator -> float32 of the same shape, `acc` cleared in place if asked."""
+    if acc.dtype != np.int32 or not acc.flags.c_contiguous:
+        raise ValueError("`acc` must be C-contiguous int32")
+    out = np.empty(acc.shape, dtype=np.float32)
+    fn = _lib().xcorr_oracle_dump
+    fn.restype = ctypes.c_longlong
+    fn.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_longlong, ctypes.c_float, ctypes.c_int]
+    if fn(acc.ctypes.data, out.ctypes.data, acc.size, float(scale), 1 if zero_acc else 0) != acc.size:
+        raise ValueError("xcorr_oracle_dump rejected its arguments")
+    return out
+
+
 def threads() -> int:
     return int(_lib().xcorr_oracle_threads())
 

@@ -292,3 +292,39 @@ def test_bad_arguments():
     with pytest.raises(ValueError):
         oracle.xcorr(x, 8, 1, 1, 8, accumulate=True)
     assert oracle.threads() >= 1
+
+
+# ---- integration dump: int32 accumulators -> float32, pinned against what IEEE-754 fixes ----
+def test_dump_exact_values_and_zeroing():
+    """Integers up to 2^24 in magnitude are exactly representable in float32: the dump of such values with scale 1
+    must reproduce them digit for digit, and power-of-two scales only change the exponent."""
+    acc = np.array([[[0, 1], [-1, 2 ** 24]], [[-(2 ** 24), 12345678], [7, -8]]], dtype=np.int32)
+    keep = acc.copy()
+    out = oracle.dump(acc, 1.0)
+    assert out.dtype == np.float32 and out.shape == acc.shape
+    assert [float(v) for v in out.reshape(-1)] == [0.0, 1.0, -1.0, 16777216.0, -16777216.0, 12345678.0, 7.0, -8.0]
+    np.testing.assert_array_equal(acc, keep)                      # zero_acc = 0 leaves the accumulator alone
+    half = oracle.dump(acc, 0.5)
+    assert [float(v) for v in half.reshape(-1)] == [0.0, 0.5, -0.5, 8388608.0, -8388608.0, 6172839.0, 3.5, -4.0]
+    out2 = oracle.dump(acc, 1.0, zero_acc=True)
+    np.testing.assert_array_equal(out2, out)
+    assert not acc.any()                                          # cleared for the next integration
+
+
+def test_dump_rounds_to_nearest_even_beyond_2_24():
+    """Worked by hand: float32 has a 24-bit significand, so above 2^24 integers are spaced 2 apart (4 above 2^25) and
+    ties go to the even significand: 2^24+1 -> 2^24, 2^24+3 -> 2^24+4, 2^25+2 -> 2^25, 2^25+6 -> 2^25+8; INT32_MAX -> 2^31."""
+    acc = np.array([2 ** 24 + 1, 2 ** 24 + 2, 2 ** 24 + 3, 2 ** 25 + 2, 2 ** 25 + 6, -(2 ** 24) - 1, 2 ** 31 - 1, -(2 ** 31)],
+                   dtype=np.int32)
+    out = oracle.dump(acc, 1.0)
+    assert [float(v) for v in out] == [16777216.0, 16777218.0, 16777220.0, 33554432.0, 33554440.0, -16777216.0,
+                                       2147483648.0, -2147483648.0]
+
+
+def test_dump_agrees_with_numpy_float32_arithmetic():
+    """Library special case: numpy's int32 -> float32 cast and float32 multiply follow the same IEEE rules."""
+    rng = np.random.default_rng(3)
+    acc = rng.integers(-2 ** 31, 2 ** 31, size=(5, 33, 2), dtype=np.int64).astype(np.int32)
+    for scale in (1.0, 1.0 / 1024, 3.0e-5):
+        exp = acc.astype(np.float32) * np.float32(scale)
+        np.testing.assert_array_equal(oracle.dump(acc, scale), exp)
