@@ -120,6 +120,18 @@ int bfXcorrGetLastCudaError(bfXcorr plan, int* cuda_error);
 int bfXcorrExecuteHost(bfXcorr plan, const void* in_host, void* out_dev, void* out_host, int accumulate,
                        void* stream);
 
+/* Integration dump -- the step after the hot path ("accumulate" hands an integration on when it is
+ * complete; integer data become floating point for the stages that follow).  Every int32 component
+ * v of the packed visibility buffer becomes   (float) v * scale   (int32 -> float32 round-to-nearest-even, then one
+ * float32 multiply) in the same [nchan][B][2] order; with zero_acc != 0 the accumulator is cleared in the same
+ * pass, so the next integration can use accumulate = 1 from its first span.
+ *   acc    : DEVICE pointer, the int32 visibility buffer of this plan (bfXcorrGetOutputBytes bytes), 16-byte aligned;
+ *            read, and written only if zero_acc != 0.
+ *   out    : DEVICE pointer, float32 buffer of the same number of bytes, 16-byte aligned, must not overlap `acc`.
+ *   stream : as bfXcorrExecute; the call only enqueues.
+ *   errors : INVALID_HANDLE; INVALID_POINTER (NULL or misaligned); DEVICE_ERROR. */
+int bfXcorrDump(bfXcorr plan, void* acc, void* out, float scale, int zero_acc, void* stream);
+
 /* Static string for a status code (never NULL). */
 const char* bfXcorrGetStatusString(int status);
 

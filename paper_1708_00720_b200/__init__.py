@@ -12,6 +12,7 @@ from .binding import (  # noqa: F401
     SIGNATURES,
     bfXcorrCreate,
     bfXcorrDestroy,
+    bfXcorrDump,
     bfXcorrExecute,
     bfXcorrExecuteHost,
     bfXcorrGetInputBytes,

@@ -35,6 +35,7 @@ SIGNATURES = {
     "bfXcorrGetLaunchCount": (_i, [_vp, _ip]),
     "bfXcorrGetLastCudaError": (_i, [_vp, _ip]),
     "bfXcorrExecuteHost": (_i, [_vp, _vp, _vp, _vp, _i, _vp]),
+    "bfXcorrDump": (_i, [_vp, _vp, _vp, ctypes.c_float, _i, _vp]),
     "bfXcorrGetStatusString": (ctypes.c_char_p, [_i]),
 }
 
@@ -85,6 +86,12 @@ def bfXcorrExecuteHost(plan: _vp, in_host_ptr: int, out_dev_ptr: int, out_host_p
                        stream: int = 0) -> None:
     _check(lib().bfXcorrExecuteHost(plan, _vp(in_host_ptr), _vp(out_dev_ptr), _vp(out_host_ptr or None),
                                     1 if accumulate else 0, _vp(stream)), "bfXcorrExecuteHost")
+
+
+def bfXcorrDump(plan: _vp, acc_ptr: int, out_ptr: int, scale: float = 1.0, zero_acc: bool = False, stream: int = 0) -> None:
+    """acc_ptr: device int32 visibilities; out_ptr: device float32 buffer of the same size."""
+    _check(lib().bfXcorrDump(plan, _vp(acc_ptr), _vp(out_ptr), ctypes.c_float(scale), 1 if zero_acc else 0, _vp(stream)),
+           "bfXcorrDump")
 
 
 def bfXcorrDestroy(plan: _vp) -> None:

@@ -10,6 +10,7 @@
 
 #include "../../include/bfxcorr.h"
 #include "xcorr_simt.cuh"
+#include "xcorr_dump.cuh"
 #include "xcorr_few.cuh"
 #include "xcorr_pair.cuh"
 #include "xcorr_common.cuh"
@@ -347,6 +348,25 @@ int bfXcorrExecuteHost(bfXcorr plan, const void* in_host, void* out_dev, void* o
         if (e == cudaSuccess) e = cudaStreamWaitEvent(s, plan->ev_d2h, 0);
     }
     if (e != cudaSuccess) return cuda_fail(plan, e);
+    return BF_XCORR_OK;
+}
+
+int bfXcorrDump(bfXcorr plan, void* acc, void* out, float scale, int zero_acc, void* stream)
+{
+    if (!valid(plan)) return BF_XCORR_INVALID_HANDLE;
+    if (!acc || !out) return BF_XCORR_INVALID_POINTER;
+    if ((reinterpret_cast<uintptr_t>(acc) & 15u) || (reinterpret_cast<uintptr_t>(out) & 15u)) return BF_XCORR_INVALID_POINTER;
+    const long long ncomp = static_cast<long long>(output_bytes(plan) / 4);
+    long long nblk = (ncomp / 4 + bfx::DUMP_THREADS - 1) / bfx::DUMP_THREADS;
+    const long long cap = 8ll * plan->num_sms;
+    if (nblk > cap) nblk = cap;
+    if (nblk < 1) nblk = 1;
+    plan->last_launch_count = 0;
+    bfx::xcorr_dump_kernel<<<dim3(static_cast<unsigned>(nblk)), bfx::DUMP_THREADS, 0, static_cast<cudaStream_t>(stream)>>>(
+        static_cast<int32_t*>(acc), static_cast<float*>(out), ncomp, scale, zero_acc ? 1 : 0);
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(plan, e);
+    plan->last_launch_count = 1;
     return BF_XCORR_OK;
 }
 

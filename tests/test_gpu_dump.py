@@ -1,0 +1,88 @@
+"""`-m gpu`: bfXcorrDump (integration dump) against the oracle, bit for bit (float32 results of a
+fixed IEEE sequence: int32 -> float32 round-to-nearest-even, one float32 multiply)."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import paper_1708_00720_b200 as bfx
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.mark.parametrize("shape", [(16, 3), (24, 1), (192, 5), (520, 2)], ids=lambda s: "n%dc%d" % s)
+@pytest.mark.parametrize("zero", [False, True])
+def test_dump_matches_oracle(shape, zero):
+    N, C = shape
+    nb = N * (N + 1) // 2
+    rng = np.random.default_rng(N + C)
+    acc = rng.integers(-2 ** 31, 2 ** 31, size=(C, nb, 2), dtype=np.int64).astype(np.int32)
+    acc.reshape(-1)[:6] = [0, 2 ** 24 + 1, 2 ** 24 + 3, -(2 ** 31), 2 ** 31 - 1, -1]   # ties and extremes
+    dev = torch.device("cuda:0")
+    plan = bfx.bfXcorrCreate(N, C, 64, 8)
+    try:
+        for scale in (1.0, 1.0 / 4096, 2.5e-4):
+            a = torch.from_numpy(acc.copy()).to(dev)
+            o = torch.full((C, nb, 2), float("nan"), dtype=torch.float32, device=dev)
+            bfx.bfXcorrDump(plan, a.data_ptr(), o.data_ptr(), scale, zero, torch.cuda.current_stream().cuda_stream)
+            assert bfx.bfXcorrGetLaunchCount(plan) == 1
+            torch.cuda.synchronize()
+            ref_acc = acc.copy()
+            exp = oracle.dump(ref_acc, scale, zero_acc=zero)
+            np.testing.assert_array_equal(o.cpu().numpy().view(np.uint32), exp.view(np.uint32))
+            np.testing.assert_array_equal(a.cpu().numpy(), ref_acc)
+    finally:
+        bfx.bfXcorrDestroy(plan)
+
+
+def test_dump_after_integration_then_next_integration_accumulates_from_zero():
+    """Two integrations of two spans each through one buffer: dump-and-clear between them."""
+    N, C, T = 136, 3, 90
+    rng = np.random.default_rng(8)
+    spans = [rng.integers(0, 256, size=(T, C, 2 * N), dtype=np.uint8) for _ in range(4)]
+    dev = torch.device("cuda:0")
+    stream = torch.cuda.current_stream().cuda_stream
+    nb = N * (N + 1) // 2
+    plan = bfx.bfXcorrCreate(N, C, T, 8)
+    try:
+        acc = torch.zeros((C, nb, 2), dtype=torch.int32, device=dev)
+        outs = []
+        for k, x in enumerate(spans):
+            xd = torch.from_numpy(x).to(dev)
+            bfx.bfXcorrExecute(plan, xd.data_ptr(), acc.data_ptr(), True, stream)   # always accumulate: buffer starts cleared
+            if k % 2 == 1:
+                o = torch.empty((C, nb, 2), dtype=torch.float32, device=dev)
+                bfx.bfXcorrDump(plan, acc.data_ptr(), o.data_ptr(), 0.5, True, stream)
+                torch.cuda.synchronize()
+                outs.append(o.cpu().numpy())
+        for k in range(2):
+            v = oracle.xcorr(spans[2 * k], N, C, T, 8)
+            oracle.xcorr(spans[2 * k + 1], N, C, T, 8, out=v, accumulate=True)
+            np.testing.assert_array_equal(outs[k], oracle.dump(v, 0.5))
+        assert int(acc.abs().max()) == 0
+    finally:
+        bfx.bfXcorrDestroy(plan)
+
+
+def test_dump_full_size_cfg3_buffer_matches_float32_cast():
+    """At BASELINE.json configs[2]'s buffer size (3.2 GB): every component equals the IEEE float32 conversion, checked
+    on the device against torch's int32 -> float32 cast and multiply (same rounding rules as the oracle's C)."""
+    from xcorr_inputs import CONFIGS
+    cfg = CONFIGS["cfg3"]
+    dev = torch.device("cuda:0")
+    if torch.cuda.mem_get_info()[0] < 4 * cfg.out_bytes:
+        pytest.skip("not enough device memory")
+    g = torch.Generator(device=dev)
+    g.manual_seed(5)
+    acc = torch.randint(-2 ** 31, 2 ** 31 - 1, (cfg.nchan, cfg.nbaselines, 2), dtype=torch.int32, device=dev, generator=g)
+    out = torch.empty(acc.shape, dtype=torch.float32, device=dev)
+    plan = bfx.bfXcorrCreate(cfg.ninputs, cfg.nchan, cfg.ntime, cfg.dtype)
+    try:
+        bfx.bfXcorrDump(plan, acc.data_ptr(), out.data_ptr(), 1.0 / 2048, False, torch.cuda.current_stream().cuda_stream)
+        torch.cuda.synchronize()
+    finally:
+        bfx.bfXcorrDestroy(plan)
+    step = cfg.nchan // 8
+    for c0 in range(0, cfg.nchan, step):
+        exp = acc[c0:c0 + step].to(torch.float32) * (1.0 / 2048)
+        assert torch.equal(out[c0:c0 + step], exp)
