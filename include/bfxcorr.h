@@ -31,7 +31,9 @@
  * work on `stream` and returns without synchronising; `in` and `out` must stay valid until the stream
  * reaches that point.  The plan owns its private device scratch (descriptors, work tables), allocated
  * by bfXcorrCreate on the CUDA device that is current at that call and released by bfXcorrDestroy.
- * A plan may be used by one host thread at a time.  Results are deterministic (integer sums).
+ * A plan may be used by one host thread at a time, and its launches must not overlap on the device (they share
+ * the plan's scheduler words, S1 ring and flags): enqueue them on one stream, or order streams with events.
+ * Results are deterministic (integer sums).
  *
  * Errors: every entry point returns a bfXcorrStatus (0 = OK); nothing aborts or throws across the ABI.
  * There is NO CPU fallback: without a compute-capability-10.x device bfXcorrCreate returns
@@ -63,9 +65,10 @@ typedef enum bfXcorrStatus_ {
     BF_XCORR_DEVICE_ERROR = 8        /* a CUDA call failed; see bfXcorrGetLastCudaError         */
 } bfXcorrStatus;
 
-/* Which kernel bfXcorrExecute launches.  TCGEN05 is the product path and the default: TMA-staged
- * int8 operands, tcgen05.mma kind::i8 with int32 accumulators held in TMEM over the whole span,
- * lower-triangle tile scheduler, span-accumulate epilogue.  SIMT is a plain CUDA-core kernel kept as
+/* Which kernel bfXcorrExecute launches.  TCGEN05 is the product path and the default: unpack-and-transpose
+ * stage, TMA-staged int8 operands, tcgen05.mma kind::i8 with int32 accumulators held in TMEM over the whole span,
+ * lower-triangle tile scheduler, span-accumulate epilogue (CTA pairs above 64 inputs, four channels per CTA up to
+ * 64 inputs: DESIGN.md section 5).  SIMT is a plain CUDA-core kernel kept as
  * an on-device cross-check of the tensor path at sizes the CPU oracle cannot reach; it is never
  * selected implicitly. */
 typedef enum bfXcorrAlgo_ {
@@ -78,7 +81,8 @@ typedef enum bfXcorrAlgo_ {
  *   *plan  : receives the handle (host pointer, must not be NULL).
  *   errors : INVALID_POINTER (plan NULL); INVALID_ARGUMENT (a dimension <= 0, or ntime > 65535);
  *            INVALID_DTYPE; UNSUPPORTED_SHAPE (ninputs * bytes_per_sample not a multiple of 16: the
- *            16-byte vector / TMA row granularity -- every BASELINE.json config satisfies it);
+ *            16-byte vector / TMA row granularity -- every BASELINE.json config satisfies it; ninputs > 32768;
+ *            or nchan * tiles-per-channel >= 2^32);
  *            UNSUPPORTED_DEVICE; MEM_ALLOC_FAILED; DEVICE_ERROR. */
 int bfXcorrCreate(bfXcorr* plan, int ninputs, int nchan, int ntime, int dtype);
 
