@@ -79,8 +79,8 @@ unsigned long long output_bytes(bfXcorr p)
 }
 
 // Where the tensor-core kernel reads its operands from: the caller's span x[t][c][...] itself (direct), or the
-// plan's channel-major int8 copy z[c][t][...] written by xcorr_relayout_kernel.  Both are addressed with the
-// same coordinates (byte in row, channel, sample); only the strides differ.
+// plan's ring of channel-major int8 slabs z[c % W][t][...] written by the relayout warps (xcorr_common.cuh).
+// Both are addressed with the same coordinates (byte in row, channel, sample); only the strides differ.
 struct OperandSource {
     const void* base;
     unsigned long long row;          // bytes per (sample, channel) row
@@ -261,7 +261,7 @@ int bfXcorrCreate(bfXcorr* plan, int ninputs, int nchan, int ntime, int dtype)
     e = cudaSuccess;
     if (e == cudaSuccess) e = cudaMalloc(reinterpret_cast<void**>(&p->d_sched), 4 * sizeof(unsigned long long));
     if (e == cudaSuccess) e = cudaMemset(p->d_sched, 0, 4 * sizeof(unsigned long long));
-    // A channel whose tiles re-read its samples is first rewritten channel-major (xcorr_relayout.cuh); with a
+    // A channel whose tiles re-read its samples is first rewritten channel-major (S1, tc_relayout_role); with a
     // single tile per channel (ninputs <= 64) every sample is read once anyway and the span is used in place.
     if (e == cudaSuccess && pair) {
         // window = channels the grid works on at once (doubled: producers run a tile or two ahead of their loads);
