@@ -153,7 +153,7 @@ __device__ __forceinline__ void tc_widen_ci4(uint32_t w, uint32_t& o0, uint32_t&
 // visibility; i0 is a multiple of 16, jb of 64) and an odd head / tail visibility goes out as a scalar store / red.
 // release_bar != 0: local shared address of the "accumulator drained" barrier to arrive on (cluster address of
 // the leader CTA's barrier in the pair kernel) once this warp's TMEM reads are done.
-template <bool SHIFT8, bool REMOTE_RELEASE = false>
+template <bool SHIFT8, bool REMOTE_RELEASE = false, int PENDING = 1>
 __device__ __forceinline__ void tc_epilogue_chunk(const TcParams& p, uint32_t lane, uint32_t tcol, uint32_t stg_buf,
                                                   int32_t* out_c, int i0, int jb, uint32_t release_bar)
 {
@@ -161,8 +161,9 @@ __device__ __forceinline__ void tc_epilogue_chunk(const TcParams& p, uint32_t la
     const int sgn = par ? -1 : 1;
     const uint32_t krow = lane >> 1;
     const uint32_t wr_off = (krow ^ ((krow >> 1) & 1)) * TC_STG_PITCH + 4 * par;
-    // the bulk group that read this staging buffer two chunks ago must be done with it
-    if (lane < 16) ptx::bulk_wait_read<1>();
+    // the bulk group that last read this staging buffer (two chunks ago with two buffers: PENDING = 1; the previous
+    // chunk with a single buffer: PENDING = 0) must be done with it
+    if (lane < 16) ptx::bulk_wait_read<PENDING>();
     __syncwarp();
 #ifdef BFX_PROBE_NO_EPI
     if (release_bar) {

@@ -21,14 +21,25 @@ constexpr int FW_KT = 64;    // samples per stage
 constexpr int FW_OP_TILE_BYTES = FW_KT * 128;             // one channel: [t][128 B] swizzled
 constexpr int FW_OP_STAGE_BYTES = FW_NC * FW_OP_TILE_BYTES;
 constexpr int FW_UNPACK_WARPS = 8;
+#ifndef BFX_FW_STG_BUFS
+#define BFX_FW_STG_BUFS 1
+#endif
+constexpr int FW_STG_BUFS = BFX_FW_STG_BUFS;          // epilogue staging buffers per warp (1: more room for span stages)
+constexpr int FW_STG_BYTES = 4 * FW_STG_BUFS * TC_STG_BUF_BYTES;
 constexpr int FW_THREADS = 256 + 32 * FW_UNPACK_WARPS;
 
 template <bool CI4>
 struct FwCfg {
     static constexpr int kRawRow = CI4 ? 64 : 128;                     // bytes of a 64-input raw row
     static constexpr int kRawStageBytes = FW_KT * FW_NC * kRawRow;     // [t][c][<= kRawRow]
-    static constexpr int kRawStages = CI4 ? 3 : 2, kOpStages = CI4 ? 3 : 2;
-    static constexpr int kSmemBytes = 1024 + kRawStages * kRawStageBytes + kOpStages * FW_OP_STAGE_BYTES + TC_STG_BYTES + 512;
+#ifndef BFX_FW_RAW4
+#define BFX_FW_RAW4 4
+#endif
+#ifndef BFX_FW_OP4
+#define BFX_FW_OP4 4
+#endif
+    static constexpr int kRawStages = CI4 ? BFX_FW_RAW4 : 2, kOpStages = CI4 ? BFX_FW_OP4 : 2;
+    static constexpr int kSmemBytes = 1024 + kRawStages * kRawStageBytes + kOpStages * FW_OP_STAGE_BYTES + FW_STG_BYTES + 512;
 };
 
 template <bool CI4>
@@ -42,7 +53,7 @@ xcorr_few_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
     const uint32_t op_base = smem_base;
     const uint32_t raw_base = op_base + S * FW_OP_STAGE_BYTES;
     const uint32_t stg_base = raw_base + R * FW_RAW_STAGE_BYTES;
-    const uint32_t bar_base = stg_base + TC_STG_BYTES;
+    const uint32_t bar_base = stg_base + FW_STG_BYTES;
     const uint32_t bar_full = bar_base;               // [S] int8 tiles written by the unpack warps
     const uint32_t bar_empty = bar_full + 8 * S;      // [S] MMAs reading the stage have completed
     const uint32_t bar_rfull = bar_empty + 8 * S;     // [R] raw bytes landed
@@ -155,7 +166,7 @@ xcorr_few_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
     } else if (warp >= 4 && warp < 8) {
         // ===================== epilogue (S4): one 64-visibility chunk per channel =====================
         const int wq = warp - 4;
-        const uint32_t stg_warp = stg_base + wq * TC_STG_WARP_BYTES;
+        const uint32_t stg_warp = stg_base + wq * FW_STG_BUFS * TC_STG_BUF_BYTES;
         const long long nbl = static_cast<long long>(p.ninputs) * (p.ninputs + 1) / 2;
         uint32_t nchunks_done = 0;
         for (uint32_t it = 0;; ++it) {
@@ -170,10 +181,10 @@ xcorr_few_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
             nch = nch > FW_NC ? FW_NC : nch;
             if (!any) nch = 0;
             for (int ch = 0; ch < nch; ++ch, ++nchunks_done) {
-                const uint32_t stg_buf = stg_warp + (nchunks_done & 1) * TC_STG_BUF_BYTES;
+                const uint32_t stg_buf = stg_warp + (nchunks_done % FW_STG_BUFS) * TC_STG_BUF_BYTES;
                 const uint32_t tcol = tmem_base + (static_cast<uint32_t>(32 * wq) << 16) + 128 * ch;
                 int32_t* const out_c = p.out + 2 * (static_cast<long long>(c0 + ch) * nbl);
-                tc_epilogue_chunk<CI4, false>(p, lane, tcol, stg_buf, out_c, 16 * wq, 0, ch == nch - 1 ? bar_tempty : 0u);
+                tc_epilogue_chunk<CI4, false, FW_STG_BUFS - 1>(p, lane, tcol, stg_buf, out_c, 16 * wq, 0, ch == nch - 1 ? bar_tempty : 0u);
             }
             if (nch == 0) {
                 ptx::tc_fence_before();
