@@ -202,29 +202,8 @@ __device__ __forceinline__ void tc_epilogue_chunk(const TcParams& p, uint32_t la
 #ifdef BFX_PROBE_NO_STORE
     return;
 #endif
-#ifdef BFX_EPI_DIRECT
-    // (alternative kept for measurement: profiles/round1.md) Write-out, coalesced: for each of the 16 rows the warp moves 2 x 32 consecutive visibilities (256 B per
-    // instruction) from the staging row to the packed triangle: plain 8-byte stores (accumulate = 0) or two
-    // 32-bit reductions performed at the L2 (accumulate != 0; the old values never travel to the SM).
-#pragma unroll 4
-    for (int r = 0; r < 16; ++r) {
-        const int i_row = i0 + r;
-        int n = i_row + 1 - jb;       // row i holds columns j <= i only (S2 masking of diagonal tiles)
-        if (i_row >= p.ninputs) n = 0;
-        int32_t* const g0 = out_c + 2 * (static_cast<long long>(i_row) * (i_row + 1) / 2 + jb);
-        const uint32_t s0 = stg_buf + (r ^ ((r >> 1) & 1)) * TC_STG_PITCH;
-#pragma unroll
-        for (int h = 0; h < 2; ++h) {
-            const int j = static_cast<int>(lane) + 32 * h;
-            if (j < n) {
-                int2 v;
-                asm volatile("ld.shared.v2.s32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(s0 + 8 * j));
-                if (p.accumulate) ptx::red_add_global_v2(g0 + 2 * j, v); else ptx::st_global_v2(g0 + 2 * j, v);
-            }
-        }
-    }
-    __syncwarp();
-#else
+    // (Coalesced st.global / red from the staging rows instead of bulk copies was measured slower: 2.38 / 3.10 vs
+    // 2.27 / 2.42 ms on cfg3, profiles/round1.md.)
     ptx::fence_proxy_async_smem();  // staging writes -> visible to the bulk-copy engine
     __syncwarp();
     if (lane < 16) {
@@ -262,7 +241,6 @@ __device__ __forceinline__ void tc_epilogue_chunk(const TcParams& p, uint32_t la
         }
         ptx::bulk_commit();
     }
-#endif
 }
 
 // ===================== relayout warps (S1: unpack-and-transpose, span -> ring z) =====================
