@@ -198,3 +198,59 @@ def test_random_shapes_sweep():
             oracle.xcorr(x, N, C, T, dtype, out=exp, accumulate=True)
         got = run_spans(xs, N, C, T, dtype, bfx.BF_XCORR_ALGO_TCGEN05)
         np.testing.assert_array_equal(got, exp, err_msg="N=%d C=%d T=%d ci%d spans=%d" % (N, C, T, dtype, nsp))
+
+
+@pytest.mark.parametrize("shape", [(16, 2, 1, 8), (16, 1, 65535, 8), (64, 3, 65535, 4), (128, 1, 4100, 8), (2048, 1, 3, 4)],
+                         ids=lambda s: "n%dc%dt%dci%d" % s)
+def test_extreme_span_lengths(shape):
+    """ntime = 1, the documented maximum 65 535 (many pipeline stages, several ring wraps), and a wide span of 3 samples."""
+    N, C, T, dtype = shape
+    x = rand_span(np.random.default_rng(T + N), T, C, N, dtype)
+    got = run_spans([x], N, C, T, dtype, bfx.BF_XCORR_ALGO_TCGEN05)
+    np.testing.assert_array_equal(got, oracle.xcorr(x, N, C, T, dtype))
+
+
+def test_many_inputs_4096_full_oracle():
+    """32 x 32 blocks of 128 inputs (528 tiles per channel): the whole packed triangle against the oracle."""
+    N, C, T = 4096, 2, 40
+    x = rand_span(np.random.default_rng(4096), T, C, N, 8)
+    got = run_spans([x], N, C, T, 8, bfx.BF_XCORR_ALGO_TCGEN05)
+    np.testing.assert_array_equal(got, oracle.xcorr(x, N, C, T, 8))
+
+
+def test_maximum_inputs_32768_sampled():
+    """The documented maximum ninputs (256 x 256 blocks, 32 896 tiles, a 4.3 GB triangle): sampled entries against the
+    oracle's per-entry evaluation, every autocorrelation against the span's power, and the last row in full."""
+    N, C, T = 32768, 1, 33
+    if torch.cuda.mem_get_info()[0] < 12 * 2 ** 30:
+        pytest.skip("needs 12 GiB of device memory")
+    rng = np.random.default_rng(32768)
+    x = rand_span(rng, T, C, N, 8)
+    dev = torch.device("cuda:0")
+    nb = N * (N + 1) // 2
+    plan = bfx.bfXcorrCreate(N, C, T, 8)
+    try:
+        out = torch.full((C, nb, 2), 0x5A5A5A5A, dtype=torch.int32, device=dev)
+        xd = torch.from_numpy(x).to(dev).reshape(-1)
+        bfx.bfXcorrExecute(plan, xd.data_ptr(), out.data_ptr(), False, torch.cuda.current_stream().cuda_stream)
+        torch.cuda.synchronize()
+    finally:
+        bfx.bfXcorrDestroy(plan)
+    i = np.concatenate([rng.integers(0, N, 4000), [0, N - 1, N - 1, 127, 128, 16383, 16384]])
+    j = np.concatenate([rng.integers(0, N, 4000), [0, 0, N - 1, 127, 127, 16383, 16383]])
+    i, j = np.maximum(i, j), np.minimum(i, j)
+    exp = oracle.xcorr_entries(x, N, C, T, 8, np.zeros_like(i), i, j)
+    k = torch.from_numpy(i * (i + 1) // 2 + j).to(dev)
+    got = out[0, k].cpu().numpy().astype(np.int64)
+    np.testing.assert_array_equal(got, exp)
+    # all autocorrelations: real, equal to each input's power
+    v = x.reshape(T, N, 2).astype(np.int8).astype(np.int64)
+    power = (v * v).sum(axis=(0, 2))
+    ii = torch.arange(N, device=dev, dtype=torch.int64)
+    autos = out[0, ii * (ii + 1) // 2 + ii].cpu().numpy()
+    np.testing.assert_array_equal(autos[:, 0], power)
+    assert not autos[:, 1].any()
+    # the last row (i = N - 1, all j) in full
+    last = out[0, (N - 1) * N // 2:(N - 1) * N // 2 + N].cpu().numpy().astype(np.int64)
+    jj = np.arange(N)
+    np.testing.assert_array_equal(last, oracle.xcorr_entries(x, N, C, T, 8, np.zeros(N, dtype=np.int64), np.full(N, N - 1), jj))
