@@ -153,13 +153,16 @@ __device__ __forceinline__ void tc_widen_ci4(uint32_t w, uint32_t& o0, uint32_t&
 // visibility; i0 is a multiple of 16, jb of 64) and an odd head / tail visibility goes out as a scalar store / red.
 // release_bar != 0: local shared address of the "accumulator drained" barrier to arrive on (cluster address of
 // the leader CTA's barrier in the pair kernel) once this warp's TMEM reads are done.
-template <bool SHIFT8, bool REMOTE_RELEASE = false, int PENDING = 1>
+template <bool SHIFT8, bool REMOTE_RELEASE = false, int PENDING = 1, bool GROUPED = false>
 __device__ __forceinline__ void tc_epilogue_chunk(const TcParams& p, uint32_t lane, uint32_t tcol, uint32_t stg_buf,
                                                   int32_t* out_c, int i0, int jb, uint32_t release_bar)
 {
-    const uint32_t par = lane & 1;                // 0: re row of its input, 1: im row
+    // Real rows / columns of the Gram matrix come interleaved (re0 im0 re1 im1 ...: the raw ci8 bytes) or, GROUPED,
+    // four at a time (re0..re3 im0..im3: what the ci4 unpack of xcorr_few.cuh writes without byte permutes); the
+    // partner lane / column holding the other part of the same input is then 4 away instead of 1.
+    const uint32_t par = GROUPED ? (lane >> 2) & 1 : lane & 1;   // 0: re row of its input, 1: im row
     const int sgn = par ? -1 : 1;
-    const uint32_t krow = lane >> 1;
+    const uint32_t krow = GROUPED ? 4 * (lane >> 3) + (lane & 3) : lane >> 1;
     const uint32_t wr_off = (krow ^ ((krow >> 1) & 1)) * TC_STG_PITCH + 4 * par;
     // the bulk group that last read this staging buffer (two chunks ago with two buffers: PENDING = 1; the previous
     // chunk with a single buffer: PENDING = 0) must be done with it
@@ -182,9 +185,11 @@ __device__ __forceinline__ void tc_epilogue_chunk(const TcParams& p, uint32_t la
         ptx::tmem_ld_wait();
 #pragma unroll
         for (int k = 0; k < 16; ++k) {
-            int ge = static_cast<int>(g[2 * k]), go = static_cast<int>(g[2 * k + 1]);
+            // columns (re_j, im_j) of visibility column j = 16 q + k
+            int ge = static_cast<int>(g[GROUPED ? 8 * (k >> 2) + (k & 3) : 2 * k]);
+            int go = static_cast<int>(g[GROUPED ? 8 * (k >> 2) + 4 + (k & 3) : 2 * k + 1]);
             if (SHIFT8) { ge >>= 8; go >>= 8; }       // G came out scaled by 16*16, exactly
-            const int v = __shfl_xor_sync(0xffffffffu, go, 1);
+            const int v = __shfl_xor_sync(0xffffffffu, go, GROUPED ? 4 : 1);
             // even lane: Re V[i][j] = G[2i][2j] + G[2i+1][2j+1]; odd lane: Im V[i][j] = G[2i+1][2j] - G[2i][2j+1]
             const int val = ge + sgn * v;
             asm volatile("st.shared.s32 [%0], %1;" ::"r"(stg_buf + wr_off + (q * 16 + k) * 8), "r"(val) : "memory");

@@ -184,7 +184,7 @@ xcorr_few_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
                 const uint32_t stg_buf = stg_warp + (nchunks_done % FW_STG_BUFS) * TC_STG_BUF_BYTES;
                 const uint32_t tcol = tmem_base + (static_cast<uint32_t>(32 * wq) << 16) + 128 * ch;
                 int32_t* const out_c = p.out + 2 * (static_cast<long long>(c0 + ch) * nbl);
-                tc_epilogue_chunk<CI4, false, FW_STG_BUFS - 1>(p, lane, tcol, stg_buf, out_c, 16 * wq, 0, ch == nch - 1 ? bar_tempty : 0u);
+                tc_epilogue_chunk<CI4, false, FW_STG_BUFS - 1, CI4>(p, lane, tcol, stg_buf, out_c, 16 * wq, 0, ch == nch - 1 ? bar_tempty : 0u);
             }
             if (nch == 0) {
                 ptx::tc_fence_before();
@@ -195,8 +195,9 @@ xcorr_few_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
         if (lane < 16) ptx::bulk_wait_read<0>();  // shared memory must outlive the bulk reads
     } else if (warp >= 8) {
         // ===================== unpack warps (S1): raw [t][c][row] nibble bytes -> per-channel int8 tiles =====================
-        // int8 tile: [t][128 B], byte 2i = re_i (ci4: << 4), byte 2i+1 = im_i (ci4: << 4), 16-byte chunks XOR-swizzled
-        // by (t & 7) exactly as TMA SWIZZLE_128B would have written them.
+        // int8 tile: [t][128 B], 16-byte chunks XOR-swizzled by (t & 7) exactly as TMA SWIZZLE_128B would have written
+        // them.  ci8: byte 2i = re_i, byte 2i+1 = im_i.  ci4: bytes 8g..8g+3 = re of inputs 4g..4g+3 (<< 4), bytes
+        // 8g+4..8g+7 = their im (<< 4).
         // lane -> (row t, 16-byte chunk qc) of one channel; a quarter-warp writes whole swizzled rows, which touches
         // every bank once; no divisions on the way.  ci4: 4 chunks of 16 samples per row, each widened to two int8
         // chunks; ci8: 8 chunks per row, copied to their swizzled place.
@@ -224,13 +225,13 @@ xcorr_few_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
                                          : "r"(rsrc + (t * FW_NC + ch) * row + qc * 16));
                             const uint32_t rowa = odst + ch * FW_OP_TILE_BYTES + t * 128;
                             if (CI4) {
+                                // grouped real embedding: the four re bytes of a word, then its four im bytes -- no byte
+                                // permutes; tc_epilogue_chunk<..., GROUPED> pairs lanes and columns 4 apart
                                 uint32_t o[8];
 #pragma unroll
                                 for (int u = 0; u < 4; ++u) {
-                                    const uint32_t hi = wv[u] & 0xF0F0F0F0u;          // 4 x (re << 4)
-                                    const uint32_t lo = (wv[u] << 4) & 0xF0F0F0F0u;   // 4 x (im << 4)
-                                    o[2 * u] = __byte_perm(hi, lo, 0x5140);           // re0 im0 re1 im1
-                                    o[2 * u + 1] = __byte_perm(hi, lo, 0x7362);       // re2 im2 re3 im3
+                                    o[2 * u] = wv[u] & 0xF0F0F0F0u;                   // re0..re3, each << 4
+                                    o[2 * u + 1] = (wv[u] << 4) & 0xF0F0F0F0u;        // im0..im3, each << 4
                                 }
                                 const uint32_t a0 = rowa + static_cast<uint32_t>((2 * qc) ^ (t & 7)) * 16;
                                 const uint32_t a1 = rowa + static_cast<uint32_t>((2 * qc + 1) ^ (t & 7)) * 16;
