@@ -13,6 +13,7 @@
 #include "xcorr_dump.cuh"
 #include "xcorr_few.cuh"
 #include "xcorr_pair.cuh"
+#include "xcorr_pair4.cuh"
 #include "xcorr_common.cuh"
 
 namespace {
@@ -95,9 +96,12 @@ OperandSource direct_source(bfXcorr p, const void* in)
     return OperandSource{in, row, row, row * static_cast<unsigned long long>(p->nchan), p->dtype == BF_XCORR_CI4};
 }
 
+// ring rows: int8 (re, im) pairs for ci8 spans, the packed bytes themselves for ci4 spans (xcorr_pair4.cuh)
+unsigned long long ring_row_bytes(bfXcorr p) { return (p->dtype == BF_XCORR_CI4 ? 1ull : 2ull) * p->ninputs; }
+
 OperandSource ring_source(bfXcorr p)
 {
-    const unsigned long long row = 2ull * p->ninputs;
+    const unsigned long long row = ring_row_bytes(p);
     return OperandSource{p->d_z, row, row * static_cast<unsigned long long>(p->ntime), row, false};
 }
 
@@ -127,7 +131,9 @@ int launch_tcgen05(bfXcorr p, const void* in, void* out, int accumulate, cudaStr
     CUtensorMap tmap;
     // operand boxes: 64 inputs x 1 channel x TC_KT samples (128 bytes of int8 pairs); few-input ci4: whole raw rows of
     // FW_NC adjacent channels x FW_KT samples
-    const int st = few ? encode_map(p, &tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, src, 1, static_cast<unsigned>(src.row),
+    const bool pair4 = pair && p->dtype == BF_XCORR_CI4;  // packed ring, unpacked in shared memory
+    const int st = pair4 ? encode_map(p, &tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, src, 1, 64u, CU_TENSOR_MAP_SWIZZLE_NONE, p->ring_w)
+                   : few ? encode_map(p, &tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, src, 1, static_cast<unsigned>(src.row),
                                     CU_TENSOR_MAP_SWIZZLE_NONE, p->nchan, bfx::FW_NC, bfx::FW_KT)
                        : encode_map(p, &tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, src, 1, CI4 ? 64u : 128u,
                                     CI4 ? CU_TENSOR_MAP_SWIZZLE_NONE : CU_TENSOR_MAP_SWIZZLE_128B, fused ? p->ring_w : p->nchan);
@@ -143,7 +149,8 @@ int launch_tcgen05(bfXcorr p, const void* in, void* out, int accumulate, cudaStr
     prm.accumulate = accumulate ? 1 : 0;
     prm.sched = p->d_sched;
     if (fused) {
-        prm.rl_ci4 = p->dtype == BF_XCORR_CI4 ? 1 : 0;
+        // ci4 spans keep their bytes in the ring (xcorr_pair4.cuh widens them in shared memory)
+        prm.rl_row_out = static_cast<int>(ring_row_bytes(p));
         prm.x = static_cast<const uint8_t*>(in);
         prm.z = p->d_z;
         prm.row_in = static_cast<int>(p->ninputs * bytes_per_sample(p->dtype));
@@ -167,8 +174,8 @@ int launch_tcgen05(bfXcorr p, const void* in, void* out, int accumulate, cudaStr
         cudaLaunchConfig_t cfg;
         std::memset(&cfg, 0, sizeof(cfg));
         cfg.gridDim = dim3(static_cast<unsigned>(2 * pairs));
-        cfg.blockDim = dim3(bfx::PR_THREADS);
-        cfg.dynamicSmemBytes = bfx::PR_SMEM_BYTES;
+        cfg.blockDim = dim3(pair4 ? bfx::P4_THREADS : bfx::PR_THREADS);
+        cfg.dynamicSmemBytes = pair4 ? bfx::P4_SMEM_BYTES : bfx::PR_SMEM_BYTES;
         cfg.stream = stream;
         cudaLaunchAttribute attr;
         attr.id = cudaLaunchAttributeClusterDimension;
@@ -177,7 +184,8 @@ int launch_tcgen05(bfXcorr p, const void* in, void* out, int accumulate, cudaStr
         attr.val.clusterDim.z = 1;
         cfg.attrs = &attr;
         cfg.numAttrs = 1;
-        e = cudaLaunchKernelEx(&cfg, bfx::xcorr_pair_kernel, tmap, prm);
+        e = pair4 ? cudaLaunchKernelEx(&cfg, bfx::xcorr_pair4_kernel, tmap, prm)
+                  : cudaLaunchKernelEx(&cfg, bfx::xcorr_pair_kernel, tmap, prm);
     } else if (few) {
         prm.ntiles = (p->nchan + bfx::FW_NC - 1) / bfx::FW_NC;
         prm.row_in = static_cast<int>(src.row);
@@ -267,7 +275,7 @@ int bfXcorrCreate(bfXcorr* plan, int ninputs, int nchan, int ntime, int dtype)
         // window = channels the grid works on at once (doubled: producers run a tile or two ahead of their loads);
         // on top of that the ring holds ~16 MiB of look-ahead, so a slab is complete long before its first tile is
         // drawn and stays L2-resident until its last tile is done
-        const unsigned long long slab = static_cast<unsigned long long>(ntime) * ninputs * 2ull;
+        const unsigned long long slab = static_cast<unsigned long long>(ntime) * ring_row_bytes(p);
         const int window = (p->num_sms / 2 + p->tiles_per_chan - 1) / p->tiles_per_chan;
         long long ahead = static_cast<long long>((16ull << 20) / slab);
         if (ahead < 2) ahead = 2;
@@ -282,6 +290,8 @@ int bfXcorrCreate(bfXcorr* plan, int ninputs, int nchan, int ntime, int dtype)
         e = cudaFuncSetAttribute(bfx::xcorr_few_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bfx::FwCfg<true>::kSmemBytes);
     if (e == cudaSuccess)
         e = cudaFuncSetAttribute(bfx::xcorr_few_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bfx::FwCfg<false>::kSmemBytes);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(bfx::xcorr_pair4_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bfx::P4_SMEM_BYTES);
     if (e == cudaSuccess)
         e = cudaFuncSetAttribute(bfx::xcorr_pair_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bfx::PR_SMEM_BYTES);
     if (e != cudaSuccess) {

@@ -51,13 +51,13 @@ struct TcParams {
     // slabs, z[c % ring_w][t][2 i + part] int8, that the relayout warps fill from the span `x`
     // ahead of the tiles being contracted.  ready[c] / done[c] count, over all launches of the
     // plan, the relayout units written for channel c / the tiles of channel c whose loads have landed.
-    int rl_ci4;
     const uint8_t* x;
     uint8_t* z;
     int row_in;             // bytes of one (t, c) row of the span
     int ring_w;
     int rl_nx, rl_units;    // 1 KiB pieces per row; relayout units per channel = rl_nx * ceil(ntime / rl_rows)
     int rl_rows;            // samples per relayout unit (a unit is about 8 KiB of span)
+    int rl_row_out;         // bytes of one (t, c) row in the ring
     unsigned long long* ready;
     unsigned long long* done;
     unsigned long long epoch;  // 1, 2, ... : launch number of this plan
@@ -129,18 +129,6 @@ struct TcRing {
         return w;
     }
 };
-
-// four ci4 bytes (re = high nibble, im = low nibble, two's complement: include/bfxcorr.h) ->
-// eight sign-extended int8: re0 im0 re1 im1 | re2 im2 re3 im3
-__device__ __forceinline__ void tc_widen_ci4(uint32_t w, uint32_t& o0, uint32_t& o1)
-{
-    const uint32_t ure = (w >> 4) & 0x0F0F0F0Fu, uim = w & 0x0F0F0F0Fu;
-    // bit 3 of a nibble set -> OR 0xF0 into its byte (bit3 * 0x1E = bits 4..7)
-    const uint32_t sre = ure | ((ure & 0x08080808u) * 0x1Eu);
-    const uint32_t sim = uim | ((uim & 0x08080808u) * 0x1Eu);
-    o0 = __byte_perm(sre, sim, 0x5140);
-    o1 = __byte_perm(sre, sim, 0x7362);
-}
 
 // ===================== one epilogue chunk (S4): 32 TMEM lanes x 128 columns -> 16 rows x 64 visibilities ==========
 // TMEM lane = real row m = 2 i + part of the A block, so lanes (2k, 2k+1) hold the re and im rows of input row
@@ -256,14 +244,12 @@ __device__ __forceinline__ void tc_relayout_role(const TcParams& p, uint32_t lan
     return;
 #endif
     // ===================== relayout warps (S1: unpack-and-transpose, span -> ring z) =====================
-    // A unit = RL_ROWS samples x one 1 KiB piece of the (t, c) row of channel cc: read with coalesced 16-byte
-    // loads (each span byte exactly once per launch), ci4 widened to sign-extended int8 pairs, written with
-    // 16-byte stores to the channel's slab.  Each warp works on its own units.
+    // A unit = rl_rows samples x one 1 KiB piece of the (t, c) row of channel cc: read with coalesced 16-byte
+    // loads (each span byte exactly once per launch) and written with 16-byte stores to the channel's slab: ci8
+    // bytes are already the int8 (re, im) pairs, ci4 bytes stay packed (xcorr_pair4.cuh widens them in shared
+    // memory).  Each warp works on its own units.
     const long long src_pitch = static_cast<long long>(p.nchan) * p.row_in;
-    const int row_out = 2 * p.ninputs;
-#ifdef BFX_L2_HINTS
-    const uint64_t pol_first = ptx::policy_evict_first(), pol_last = ptx::policy_evict_last();  // span: once; ring: keep
-#endif
+    const int row_out = p.rl_row_out;  // bytes of one (t, c) row in the ring: 2 N (int8 pairs) or N (packed ci4)
     auto do_unit = [&](int cc, int u) {
         if (cc >= p.ring_w) {
             // the slab is still owned by channel cc - ring_w until all of its tiles have loaded their operands
@@ -284,7 +270,7 @@ __device__ __forceinline__ void tc_relayout_role(const TcParams& p, uint32_t lan
         const int total = nt * nv;
         const int nv_shift = (nv & (nv - 1)) == 0 ? 31 - __clz(nv) : -1;  // rows are usually 64 vectors: avoid the division
         const uint8_t* src = p.x + (static_cast<long long>(t0) * p.nchan + cc) * p.row_in + xb0;
-        uint8_t* dst = p.z + (static_cast<long long>(cc % p.ring_w) * p.ntime + t0) * row_out + (p.rl_ci4 ? 2 * xb0 : xb0);
+        uint8_t* dst = p.z + (static_cast<long long>(cc % p.ring_w) * p.ntime + t0) * row_out + xb0;
         constexpr int U = 16;
         for (int base = static_cast<int>(lane); base < total; base += U * 32) {
             uint4 v[U];
@@ -299,20 +285,8 @@ __device__ __forceinline__ void tc_relayout_role(const TcParams& p, uint32_t lan
                 const int idx = base + 32 * k;
                 const int r = nv_shift >= 0 ? idx >> nv_shift : idx / nv;
                 const int vi = idx - r * nv;
-                if (idx < total) {
-                    if (p.rl_ci4) {
-                        uint8_t* d = dst + static_cast<long long>(r) * row_out + vi * 32;
-                        uint4 a, b;
-                        tc_widen_ci4(v[k].x, a.x, a.y);
-                        tc_widen_ci4(v[k].y, a.z, a.w);
-                        tc_widen_ci4(v[k].z, b.x, b.y);
-                        tc_widen_ci4(v[k].w, b.z, b.w);
-                        ptx::st_global_v4(d, a);
-                        ptx::st_global_v4(d + 16, b);
-                    } else {
-                        ptx::st_global_v4(dst + static_cast<long long>(r) * row_out + vi * 16, v[k]);
-                    }
-                }
+                // (eviction hints on these loads / stores were measured harmful: cfg3 accumulate span 2.49 vs 2.34 ms)
+                if (idx < total) ptx::st_global_v4(dst + static_cast<long long>(r) * row_out + vi * 16, v[k]);
             }
         }
         // publish: every lane's stores are ordered before lane 0's release by the warp barrier (the release is
