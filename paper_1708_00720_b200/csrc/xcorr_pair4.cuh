@@ -24,7 +24,7 @@ constexpr int P4_RAW_BOX = TC_KT * 64;               // one raw box: TC_KT rows 
 constexpr int P4_RAW_STAGE = 2 * P4_RAW_BOX;         // A-half, B-half
 constexpr int P4_OP_STAGE = 2 * TC_BOX_BYTES;        // the same, widened
 #ifndef BFX_P4_RAW
-#define BFX_P4_RAW 5
+#define BFX_P4_RAW 6
 #endif
 #ifndef BFX_P4_OP
 #define BFX_P4_OP 3
