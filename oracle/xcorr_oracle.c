@@ -149,7 +149,6 @@ long long xcorr_oracle(const uint8_t* in, int32_t* out, int ninputs, int nchan, 
     return nwrap;
 }
 
-/* Number of threads the span routine will use (1 when built without OpenMP). */
 /* Integration dump (the paper's accumulate block hands an integration on when it is
  * complete, and its pipelines convert integer data to floating point for the stages that follow,
  * PAPER.md:549): every int32 component v of the packed visibility buffer becomes the float32
@@ -168,6 +167,53 @@ long long xcorr_oracle_dump(int32_t* acc, float* out, long long ncomponents, flo
     return ncomponents;
 }
 
+/* Beamformer on the same span (the GPU stage the paper's deployment runs on the
+ * "4+4 complex signed integers"; a "phase-and-sum" of all inputs per beam):
+ *
+ *   for every sample t, channel c and beam k
+ *       b[t][c][k] = sum over inputs i of   w[c][k][i] * x[t][c][i]           (complex product, no conjugate)
+ *         .re = sum_i ( wr*xr - wi*xi )
+ *         .im = sum_i ( wr*xi + wi*xr )
+ *       out[t][c][k] = b            (int32 re, int32 im; sums taken in int64 and truncated to 32 bits)
+ *
+ * x as above (ci4 or ci8).  Weights w: dense [nchan][nbeam][ninputs], input fastest, always 8+8 bit: byte 0 = re,
+ * byte 1 = im, int8.  The code -128 is legal for re; for im it is outside the domain (the quantised weights are
+ * symmetric, [-127, 127]) and the routine rejects it (returns -2).
+ * Returns the number of sums that did not fit in int32 (0 for every legal input: 2 * 32768 * 128 * 128 < 2^31
+ * holds up to 32768 inputs), -1 on bad arguments. */
+long long xcorr_oracle_beamform(const uint8_t* in, const uint8_t* w, int32_t* out, int ninputs, int nchan,
+                                int ntime, int nbeam, int dtype)
+{
+    const long long N = ninputs, C = nchan, T = ntime, K = nbeam;
+    long long nwrap = 0, q;
+    if (!in || !w || !out || N <= 0 || C <= 0 || T <= 0 || K <= 0 || (dtype != 4 && dtype != 8)) return -1;
+    for (q = 0; q < C * K * N; ++q)
+        if ((int8_t)w[2 * q + 1] == -128) return -2;
+#ifdef _OPENMP
+#pragma omp parallel for collapse(2) reduction(+ : nwrap) schedule(static)
+#endif
+    for (long long t = 0; t < T; ++t) {
+        for (long long c = 0; c < C; ++c) {
+            for (long long k = 0; k < K; ++k) {
+                int64_t sr = 0, si = 0;
+                for (long long i = 0; i < N; ++i) {
+                    int xr, xi;
+                    const uint8_t* wp = w + 2 * ((c * K + k) * N + i);
+                    const int wr = (int8_t)wp[0], wi = (int8_t)wp[1];
+                    decode_sample(in, dtype, N, C, t, c, i, &xr, &xi);
+                    sr += (int64_t)(wr * xr - wi * xi);
+                    si += (int64_t)(wr * xi + wi * xr);
+                }
+                nwrap += !fits32(sr) + !fits32(si);
+                out[2 * ((t * C + c) * K + k) + 0] = (int32_t)(uint32_t)(uint64_t)sr;
+                out[2 * ((t * C + c) * K + k) + 1] = (int32_t)(uint32_t)(uint64_t)si;
+            }
+        }
+    }
+    return nwrap;
+}
+
+/* Number of threads the span routines will use (1 when built without OpenMP). */
 #ifdef _OPENMP
 #include <omp.h>
 int xcorr_oracle_threads(void) { return omp_get_max_threads(); }

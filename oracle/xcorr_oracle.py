@@ -126,6 +126,25 @@ def dump(acc: np.ndarray, scale: float = 1.0, zero_acc: bool = False) -> np.ndar
     return out
 
 
+def beamform(x: np.ndarray, w: np.ndarray, ninputs: int, nchan: int, ntime: int, nbeam: int, dtype: int,
+             return_nwrap: bool = False):
+    """Phase-and-sum beamformer: span x, ci8 weights [nchan][nbeam][ninputs] -> int32 [ntime][nchan][nbeam][2]."""
+    x = _check_in(x, ninputs, nchan, ntime, dtype)
+    w = np.ascontiguousarray(w).view(np.uint8).reshape(-1)
+    if w.size != nchan * nbeam * ninputs * 2:
+        raise ValueError("weights have %d bytes, expected %d" % (w.size, nchan * nbeam * ninputs * 2))
+    out = np.empty((ntime, nchan, nbeam, 2), dtype=np.int32)
+    fn = _lib().xcorr_oracle_beamform
+    fn.restype = ctypes.c_longlong
+    fn.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p] + [ctypes.c_int] * 5
+    nwrap = fn(x.ctypes.data, w.ctypes.data, out.ctypes.data, ninputs, nchan, ntime, nbeam, dtype)
+    if nwrap == -2:
+        raise ValueError("weight imaginary part -128 is outside the domain")
+    if nwrap < 0:
+        raise ValueError("xcorr_oracle_beamform rejected its arguments")
+    return (out, int(nwrap)) if return_nwrap else out
+
+
 def threads() -> int:
     return int(_lib().xcorr_oracle_threads())
 

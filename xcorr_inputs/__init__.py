@@ -18,4 +18,5 @@ from .gen import (  # noqa: F401
     generate_channel_slab,
     gauss_thresholds,
     tone_offsets,
+    generate_weights,
 )
