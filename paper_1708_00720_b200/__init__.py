@@ -1,6 +1,6 @@
 """paper_1708_00720_b200 -- B200-native X-engine (cross-multiply-accumulate) of a Bifrost-style
 correlator back end (arXiv:1708.00720).  The product is the C-ABI library declared in
-include/bfxcorr.h (built from csrc/ into libbfxcorr.so); this package is its thin ctypes binding.
+include/bfxcorr.h and include/bfbeamform.h (built from csrc/ into libbfxcorr.so); this package is its thin ctypes binding.
 """
 from .binding import (  # noqa: F401
     BF_XCORR_ALGO_SIMT,
@@ -10,6 +10,14 @@ from .binding import (  # noqa: F401
     BF_XCORR_OK,
     BfXcorrError,
     SIGNATURES,
+    bfBeamformCreate,
+    bfBeamformDestroy,
+    bfBeamformExecute,
+    bfBeamformGetInputBytes,
+    bfBeamformGetLastCudaError,
+    bfBeamformGetOutputBytes,
+    bfBeamformGetWeightBytes,
+    bfBeamformSetWeights,
     bfXcorrCreate,
     bfXcorrDestroy,
     bfXcorrDump,

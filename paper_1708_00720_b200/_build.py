@@ -47,12 +47,12 @@ def needs_build() -> bool:
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    """Compile csrc/bfxcorr.cu -> libbfxcorr.so; returns the library path."""
+    """Compile csrc/bfxcorr.cu and csrc/bfbeamform.cu -> libbfxcorr.so; returns the library path."""
     if not force and not needs_build():
         return LIB_PATH
     tmp = LIB_PATH + ".tmp%d" % os.getpid()
     cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + [
-        "-I", INCLUDE, "-o", tmp, os.path.join(CSRC, "bfxcorr.cu")]
+        "-I", INCLUDE, "-o", tmp, os.path.join(CSRC, "bfxcorr.cu"), os.path.join(CSRC, "bfbeamform.cu")]
     res = subprocess.run(cmd, capture_output=True, text=True)
     if res.returncode != 0:
         raise RuntimeError("nvcc failed:\n%s\n%s" % (" ".join(cmd), res.stderr))

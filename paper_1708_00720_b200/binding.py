@@ -23,7 +23,7 @@ _i = ctypes.c_int
 _ullp = ctypes.POINTER(ctypes.c_ulonglong)
 _ip = ctypes.POINTER(ctypes.c_int)
 
-# name -> (restype, argtypes); mirrors include/bfxcorr.h one to one
+# name -> (restype, argtypes); mirrors include/bfxcorr.h and include/bfbeamform.h one to one
 SIGNATURES = {
     "bfXcorrCreate": (_i, [ctypes.POINTER(_vp), _i, _i, _i, _i]),
     "bfXcorrExecute": (_i, [_vp, _vp, _vp, _i, _vp]),
@@ -37,6 +37,15 @@ SIGNATURES = {
     "bfXcorrExecuteHost": (_i, [_vp, _vp, _vp, _vp, _i, _vp]),
     "bfXcorrDump": (_i, [_vp, _vp, _vp, ctypes.c_float, _i, _vp]),
     "bfXcorrGetStatusString": (ctypes.c_char_p, [_i]),
+    # include/bfbeamform.h
+    "bfBeamformCreate": (_i, [ctypes.POINTER(_vp), _i, _i, _i, _i, _i]),
+    "bfBeamformSetWeights": (_i, [_vp, _vp, _vp]),
+    "bfBeamformExecute": (_i, [_vp, _vp, _vp, _vp]),
+    "bfBeamformDestroy": (_i, [_vp]),
+    "bfBeamformGetInputBytes": (_i, [_vp, _ullp]),
+    "bfBeamformGetWeightBytes": (_i, [_vp, _ullp]),
+    "bfBeamformGetOutputBytes": (_i, [_vp, _ullp]),
+    "bfBeamformGetLastCudaError": (_i, [_vp, _ip]),
 }
 
 _LIB: Optional[ctypes.CDLL] = None
@@ -129,4 +138,42 @@ def bfXcorrGetLaunchCount(plan: _vp) -> int:
 def bfXcorrGetLastCudaError(plan: _vp) -> int:
     v = ctypes.c_int(0)
     _check(lib().bfXcorrGetLastCudaError(plan, ctypes.byref(v)), "bfXcorrGetLastCudaError")
+    return int(v.value)
+
+
+# ---- include/bfbeamform.h ---------------------------------------------------------------------
+def bfBeamformCreate(ninputs: int, nchan: int, ntime: int, nbeam: int, dtype: int) -> _vp:
+    plan = _vp()
+    _check(lib().bfBeamformCreate(ctypes.byref(plan), ninputs, nchan, ntime, nbeam, dtype), "bfBeamformCreate")
+    return plan
+
+
+def bfBeamformSetWeights(plan: _vp, weights_ptr: int, stream: int = 0) -> None:
+    """weights_ptr: device address of the ci8 weights [nchan][nbeam][ninputs]; synchronises `stream`."""
+    _check(lib().bfBeamformSetWeights(plan, _vp(weights_ptr), _vp(stream)), "bfBeamformSetWeights")
+
+
+def bfBeamformExecute(plan: _vp, in_ptr: int, out_ptr: int, stream: int = 0) -> None:
+    _check(lib().bfBeamformExecute(plan, _vp(in_ptr), _vp(out_ptr), _vp(stream)), "bfBeamformExecute")
+
+
+def bfBeamformDestroy(plan: _vp) -> None:
+    _check(lib().bfBeamformDestroy(plan), "bfBeamformDestroy")
+
+
+def bfBeamformGetInputBytes(plan: _vp) -> int:
+    return _get_ull("bfBeamformGetInputBytes", plan)
+
+
+def bfBeamformGetWeightBytes(plan: _vp) -> int:
+    return _get_ull("bfBeamformGetWeightBytes", plan)
+
+
+def bfBeamformGetOutputBytes(plan: _vp) -> int:
+    return _get_ull("bfBeamformGetOutputBytes", plan)
+
+
+def bfBeamformGetLastCudaError(plan: _vp) -> int:
+    v = ctypes.c_int(0)
+    _check(lib().bfBeamformGetLastCudaError(plan, ctypes.byref(v)), "bfBeamformGetLastCudaError")
     return int(v.value)

@@ -1,0 +1,335 @@
+// beamform.cuh -- phase-and-sum beamformer on the span x[t][c][i] (include/bfbeamform.h).
+//
+// Per channel c it is the dense contraction  b[t][k] = sum_i w[c][k][i] x[t][c][i]  over the INPUT axis, so, unlike
+// the X-engine, the span rows are already the K-major operand: a row x[t][c][0..N) of ci8 samples is, byte for byte,
+// the int8 row a[t][0..2N) with a[2i] = re_i, a[2i+1] = im_i, and the plan holds, per channel, two int8 rows per beam
+//     W[2k  ][2i] =  wr   W[2k  ][2i+1] = -wi          ->  D[t][2k]   = Re b[t][k]
+//     W[2k+1][2i] =  wi   W[2k+1][2i+1] =  wr          ->  D[t][2k+1] = Im b[t][k]
+// (bfBeamformSetWeights; kind::i8 cannot negate an operand, hence the im != -128 domain).  ci4 rows are widened
+// on chip as in xcorr_pair4.cuh: each 32-bit word of 4 samples becomes the 4 re bytes (<< 4) then the 4 im bytes
+// (<< 4), the weight rows are stored in the same grouped order, and the factor 16 is shifted out exactly in the
+// epilogue.  Every sample is used once, so the span is consumed in place: no ring, no relayout.
+//
+// Work unit: 128 samples x 1 channel (MMA M = 128 samples, N = 2 nbeam rounded up to 16, K = the input axis in
+// stages of 128 span bytes).  Units are dealt round-robin in groups of `group` adjacent channels x all sample blocks,
+// so the CTAs of one wave read adjacent channels of the same samples (whole DRAM pages) and a group's weights stay
+// in the L2 while its sample blocks go by.
+//
+// Roles (512 threads, one CTA per SM): warp 0 weight producer (TMA, 128B-swizzled K-major boxes), warp 1 MMA issuer,
+// warp 2 TMEM allocator, warps 4..7 epilogue (TMEM -> registers -> global, one sample row per thread), warps 8..15
+// loaders: coalesced 16-byte span loads, two stages in flight per thread, written (ci4: widened) into the
+// 128B-swizzled K-major layout the UMMA descriptor expects.
+#pragma once
+#include <cstdint>
+#include <cuda.h>
+#include "ptx_sm100.cuh"
+
+namespace bfx {
+
+constexpr int BM_MT = 128;             // samples per unit
+constexpr int BM_LOAD_WARPS = 8;
+constexpr int BM_THREADS = 256 + 32 * BM_LOAD_WARPS;
+constexpr int BM_MAX_STAGES = 8;
+constexpr int BM_DEPTH = 2;            // span stages in flight per loader thread
+constexpr int BM_SMEM_MAX = 232448 - 1024;
+
+struct BmParams {
+    const uint8_t* x;
+    int32_t* out;
+    int ninputs, nchan, ntime, nbeam;
+    int row_in;      // bytes of one (t, c) row of the span
+    int nb2;         // MMA N: 2 * nbeam rounded up to a multiple of 16
+    int nks;         // K stages: ceil(row_in / 128)
+    int ntb;         // sample blocks: ceil(ntime / 128)
+    int group;       // adjacent channels per scheduling group
+    int stages;      // pipeline depth
+    long long nunits;
+};
+
+// the (sample block, channel) of unit u: groups of `group` channels, sample blocks inside a group, channels fastest
+struct BmUnit {
+    int c, t0;
+};
+__device__ __forceinline__ BmUnit bm_decode(const BmParams& p, long long u)
+{
+    const long long per = static_cast<long long>(p.group) * p.ntb;
+    const int cg = static_cast<int>(u / per);
+    const int r = static_cast<int>(u - cg * per);
+    int gl = p.nchan - cg * p.group;
+    gl = gl > p.group ? p.group : gl;
+    const int tb = r / gl;
+    return BmUnit{cg * p.group + (r - tb * gl), tb * BM_MT};
+}
+
+// UMMA shared-memory descriptor, K-major, SWIZZLE_128B: rows of 128 bytes, 8-row atoms 1024 bytes apart
+__device__ __forceinline__ uint64_t bm_smem_desc(uint32_t saddr)
+{
+    uint64_t d = 0;
+    d |= static_cast<uint64_t>((saddr >> 4) & 0x3FFF);
+    d |= static_cast<uint64_t>(1) << 16;
+    d |= static_cast<uint64_t>((1024u >> 4) & 0x3FFF) << 32;
+    d |= static_cast<uint64_t>(1) << 46;
+    d |= static_cast<uint64_t>(2) << 61;
+    return d;
+}
+
+// UMMA instruction descriptor: dense, D = S32, A = B = signed int8, both K-major
+__host__ __device__ constexpr uint32_t bm_instr_desc(int m, int n)
+{
+    return (2u << 4) | (1u << 7) | (1u << 10) | (static_cast<uint32_t>(n >> 3) << 17) | (static_cast<uint32_t>(m >> 4) << 24);
+}
+
+template <bool CI4>
+__global__ void __launch_bounds__(BM_THREADS, 1)
+beamform_kernel(const __grid_constant__ CUtensorMap wmap, const BmParams p)
+{
+    constexpr int KS = CI4 ? 256 : 128;        // int8 K bytes per stage (128 span bytes)
+    constexpr int KH = KS / 128;               // 128-byte K tiles per stage
+    constexpr int A_TILE = BM_MT * 128;
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
+    const uint32_t w_tile = static_cast<uint32_t>(p.nb2) * 128u;
+    const uint32_t stage_bytes = KH * (A_TILE + w_tile);
+    const int S = p.stages;
+    const uint32_t bar_base = smem_base + S * stage_bytes;
+    const uint32_t bar_full = bar_base;                          // [S] span tile written + weight boxes landed
+    const uint32_t bar_empty = bar_full + 8 * BM_MAX_STAGES;     // [S] MMAs reading the stage have completed
+    const uint32_t bar_tfull = bar_empty + 8 * BM_MAX_STAGES;    // [2] accumulator complete
+    const uint32_t bar_tempty = bar_tfull + 16;                  // [2] accumulator drained
+    const uint32_t tmem_slot = bar_tempty + 16;
+
+    const int warp = threadIdx.x >> 5;
+    const uint32_t lane = ptx::lane_id();
+
+    if (warp == 0 && lane == 0) {
+        ptx::prefetch_tensormap(&wmap);
+        for (int s = 0; s < S; ++s) {
+            ptx::mbar_init(bar_full + 8 * s, BM_LOAD_WARPS + 1);
+            ptx::mbar_init(bar_empty + 8 * s, 1);
+        }
+        for (int b = 0; b < 2; ++b) {
+            ptx::mbar_init(bar_tfull + 8 * b, 1);
+            ptx::mbar_init(bar_tempty + 8 * b, 4);
+        }
+        ptx::fence_barrier_init();
+    }
+    if (warp == 2) {
+        ptx::tmem_alloc<1>(tmem_slot, 512);
+        ptx::tmem_relinquish<1>();
+    }
+    ptx::tc_fence_before();
+    __syncthreads();
+    ptx::tc_fence_after();
+    uint32_t tmem_base;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
+
+    const long long u0 = blockIdx.x, ustep = gridDim.x;
+
+    if (warp == 0) {
+        // ===================== weight producer (converged warp, lane 0 issues) =====================
+        uint32_t stage = 0, phase = 0;
+        for (long long u = u0; u < p.nunits; u += ustep) {
+            const BmUnit un = bm_decode(p, u);
+            for (int ks = 0; ks < p.nks; ++ks) {
+                ptx::mbar_wait(bar_empty + 8 * stage, phase ^ 1);
+                if (lane == 0) {
+                    const uint32_t dst = smem_base + stage * stage_bytes + KH * A_TILE;
+                    ptx::mbar_expect_tx(bar_full + 8 * stage, KH * w_tile);
+#pragma unroll
+                    for (int h = 0; h < KH; ++h)
+                        ptx::tma_load_2d(dst + h * w_tile, &wmap, bar_full + 8 * stage, ks * KS + h * 128, un.c * p.nb2);
+                }
+                __syncwarp();
+                if (++stage == static_cast<uint32_t>(S)) { stage = 0; phase ^= 1; }
+            }
+        }
+    } else if (warp == 1) {
+        // ===================== MMA issuer (converged warp, lane 0 issues) =====================
+        uint32_t stage = 0, phase = 0, it = 0;
+        const uint32_t idesc = bm_instr_desc(BM_MT, p.nb2);
+        for (long long u = u0; u < p.nunits; u += ustep, ++it) {
+            const uint32_t b = it & 1;
+            ptx::mbar_wait(bar_tempty + 8 * b, ((it >> 1) & 1) ^ 1);
+            ptx::tc_fence_after();
+            for (int ks = 0; ks < p.nks; ++ks) {
+                ptx::mbar_wait(bar_full + 8 * stage, phase);
+                ptx::tc_fence_after();
+                if (lane == 0) {
+                    const uint32_t abase = smem_base + stage * stage_bytes;
+                    const uint32_t wbase = abase + KH * A_TILE;
+#pragma unroll
+                    for (int h = 0; h < KH; ++h) {
+                        const uint64_t adesc = bm_smem_desc(abase + h * A_TILE);
+                        const uint64_t bdesc = bm_smem_desc(wbase + h * w_tile);
+#pragma unroll
+                        for (int k = 0; k < 4; ++k)
+                            ptx::mma_i8<1>(tmem_base + 256 * b, adesc + 2u * k, bdesc + 2u * k, idesc, (ks | h | k) != 0 ? 1u : 0u);
+                    }
+                    ptx::mma_commit(bar_empty + 8 * stage);
+                }
+                __syncwarp();
+                if (++stage == static_cast<uint32_t>(S)) { stage = 0; phase ^= 1; }
+            }
+            if (lane == 0) ptx::mma_commit(bar_tfull + 8 * b);
+            __syncwarp();
+        }
+    } else if (warp >= 4 && warp < 8) {
+        // ===================== epilogue: one sample row per thread =====================
+        const int wq = warp - 4;
+        uint32_t it = 0;
+        const bool vec4 = (p.nbeam & 1) == 0;
+        for (long long u = u0; u < p.nunits; u += ustep, ++it) {
+            const BmUnit un = bm_decode(p, u);
+            const uint32_t b = it & 1;
+            ptx::mbar_wait(bar_tfull + 8 * b, (it >> 1) & 1);
+            ptx::tc_fence_after();
+            const int t = un.t0 + 32 * wq + static_cast<int>(lane);
+            int32_t* const orow = p.out + 2 * ((static_cast<long long>(t) * p.nchan + un.c) * p.nbeam);
+            for (int col = 0; col < 2 * p.nbeam; col += 32) {
+                uint32_t r[32];
+                ptx::tmem_ld_32x32b_x32(tmem_base + (static_cast<uint32_t>(32 * wq) << 16) + 256 * b + col, r);
+                ptx::tmem_ld_wait();
+                if (CI4) {
+#pragma unroll
+                    for (int j = 0; j < 32; ++j) r[j] = static_cast<uint32_t>(static_cast<int32_t>(r[j]) >> 4);
+                }
+                if (t < p.ntime) {
+                    if (vec4) {
+#pragma unroll
+                        for (int j = 0; j < 32; j += 4)
+                            if (col + j < 2 * p.nbeam)
+                                ptx::st_global_v4(reinterpret_cast<uint8_t*>(orow + col + j), make_uint4(r[j], r[j + 1], r[j + 2], r[j + 3]));
+                    } else {
+#pragma unroll
+                        for (int j = 0; j < 32; j += 2)
+                            if (col + j < 2 * p.nbeam)
+                                ptx::st_global_v2(orow + col + j, make_int2(static_cast<int>(r[j]), static_cast<int>(r[j + 1])));
+                    }
+                }
+            }
+            ptx::tc_fence_before();
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(bar_tempty + 8 * b);
+        }
+    } else if (warp >= 8) {
+        // ===================== loaders: span rows -> swizzled K-major int8 tiles =====================
+        // vector v = i * 256 + tid of a stage: sample row v >> 3, 16-byte chunk v & 7 of the row's 128 span bytes;
+        // eight lanes read one whole 128-byte line and (ci8) write one whole swizzled row
+        const int tid = static_cast<int>(threadIdx.x) - 256;
+        const int chunk = tid & 7;
+        struct It {
+            long long u;
+            int ks, c, t0;
+        };
+        It li{u0, 0, 0, 0}, si{u0, 0, 0, 0};
+        if (u0 < p.nunits) {
+            const BmUnit un = bm_decode(p, u0);
+            li.c = si.c = un.c;
+            li.t0 = si.t0 = un.t0;
+        }
+        auto advance = [&](It& a) {
+            if (++a.ks == p.nks) {
+                a.ks = 0;
+                a.u += ustep;
+                if (a.u < p.nunits) {
+                    const BmUnit un = bm_decode(p, a.u);
+                    a.c = un.c;
+                    a.t0 = un.t0;
+                }
+            }
+        };
+        uint4 buf[BM_DEPTH][4];
+        auto issue = [&](const It& a, uint4* v) {
+            const int kbyte = a.ks * 128 + chunk * 16;
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const int t = a.t0 + i * 32 + (tid >> 3);
+                v[i] = make_uint4(0u, 0u, 0u, 0u);
+                if (a.u < p.nunits && t < p.ntime && kbyte < p.row_in)
+                    v[i] = ptx::ld_global_stream_v4(p.x + (static_cast<long long>(t) * p.nchan + a.c) * p.row_in + kbyte);
+            }
+        };
+#pragma unroll
+        for (int d = 0; d < BM_DEPTH; ++d) {
+            issue(li, buf[d]);
+            advance(li);
+        }
+        uint32_t stage = 0, phase = 0;
+        while (si.u < p.nunits) {
+#pragma unroll
+            for (int d = 0; d < BM_DEPTH; ++d) {
+                if (si.u < p.nunits) {
+                    ptx::mbar_wait(bar_empty + 8 * stage, phase ^ 1);
+                    const uint32_t abase = smem_base + stage * stage_bytes;
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+                        const int rowi = i * 32 + (tid >> 3);
+                        const uint4 w = buf[d][i];
+                        const uint32_t rowa = abase + rowi * 128;
+                        if (CI4) {
+                            // 16 packed samples -> chunks 2 * chunk and 2 * chunk + 1 of the 256-byte int8 row
+                            const uint32_t tile = rowa + (chunk >> 2) * A_TILE;
+                            const uint32_t j0 = static_cast<uint32_t>(2 * chunk) & 7u;
+                            const uint32_t a0 = tile + ((j0 ^ (rowi & 7)) << 4), a1 = tile + (((j0 + 1) ^ (rowi & 7)) << 4);
+                            asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(a0), "r"(w.x & 0xF0F0F0F0u),
+                                         "r"((w.x << 4) & 0xF0F0F0F0u), "r"(w.y & 0xF0F0F0F0u), "r"((w.y << 4) & 0xF0F0F0F0u)
+                                         : "memory");
+                            asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(a1), "r"(w.z & 0xF0F0F0F0u),
+                                         "r"((w.z << 4) & 0xF0F0F0F0u), "r"(w.w & 0xF0F0F0F0u), "r"((w.w << 4) & 0xF0F0F0F0u)
+                                         : "memory");
+                        } else {
+                            const uint32_t a0 = rowa + ((static_cast<uint32_t>(chunk) ^ (rowi & 7)) << 4);
+                            asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(a0), "r"(w.x), "r"(w.y), "r"(w.z), "r"(w.w) : "memory");
+                        }
+                    }
+                    ptx::fence_proxy_async_smem();  // generic-proxy stores -> visible to the tensor core (async proxy)
+                    __syncwarp();
+                    if (lane == 0) ptx::mbar_arrive(bar_full + 8 * stage);
+                    if (++stage == static_cast<uint32_t>(S)) { stage = 0; phase ^= 1; }
+                    issue(li, buf[d]);
+                    advance(li);
+                    advance(si);
+                }
+            }
+        }
+    }
+
+    ptx::tc_fence_before();
+    __syncthreads();
+    if (warp == 2) ptx::tmem_dealloc<1>(tmem_base, 512);
+}
+
+// bfBeamformSetWeights: w[c][k][i] (ci8) -> W[c][n][kk] int8, n = 2k + part of b, kk in the order the loaders write
+// the span bytes (header comment); rows n >= 2 nbeam and columns beyond the inputs are zero.  *bad |= 1 if an
+// imaginary part is -128.
+template <bool CI4>
+__global__ void beamform_weights_kernel(const int8_t* __restrict__ w, int8_t* __restrict__ wp, int ninputs, int nchan, int nbeam,
+                                        int nb2, int kp, int* bad)
+{
+    const long long total = static_cast<long long>(nchan) * nb2 * kp;
+    for (long long q = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x; q < total;
+         q += static_cast<long long>(gridDim.x) * blockDim.x) {
+        const int kk = static_cast<int>(q % kp);
+        const long long cn = q / kp;
+        const int n = static_cast<int>(cn % nb2), c = static_cast<int>(cn / nb2);
+        const int k = n >> 1, bpart = n & 1;
+        int i, xpart;
+        if (CI4) {
+            i = 4 * (kk >> 3) + (kk & 3);
+            xpart = (kk >> 2) & 1;
+        } else {
+            i = kk >> 1;
+            xpart = kk & 1;
+        }
+        int v = 0;
+        if (k < nbeam && i < ninputs) {
+            const int8_t* s = w + 2 * ((static_cast<long long>(c) * nbeam + k) * ninputs + i);
+            const int wr = s[0], wi = s[1];
+            if (wi == -128) atomicOr(bad, 1);
+            v = bpart == 0 ? (xpart == 0 ? wr : -wi) : (xpart == 0 ? wi : wr);
+        }
+        wp[q] = static_cast<int8_t>(v);
+    }
+}
+
+}  // namespace bfx

@@ -10,18 +10,21 @@ import pytest
 import paper_1708_00720_b200 as bfx
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
-HEADER = os.path.join(ROOT, "include", "bfxcorr.h")
+HEADERS = [os.path.join(ROOT, "include", n) for n in sorted(os.listdir(os.path.join(ROOT, "include"))) if n.endswith(".h")]
 
 
 def _declared_functions():
-    src = open(HEADER).read()
-    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    return sorted(set(re.findall(r"\b(bfXcorr[A-Z]\w*)\s*\(", src)))
+    names = set()
+    for header in HEADERS:
+        src = open(header).read()
+        src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+        names.update(re.findall(r"\b(bf(?:Xcorr|Beamform)[A-Z]\w*)\s*\(", src))
+    return sorted(names)
 
 
 def test_header_declares_the_north_star_entry_points():
     names = _declared_functions()
-    for must in ("bfXcorrCreate", "bfXcorrExecute", "bfXcorrDestroy"):
+    for must in ("bfXcorrCreate", "bfXcorrExecute", "bfXcorrDestroy", "bfBeamformCreate", "bfBeamformExecute"):
         assert must in names
 
 
@@ -54,6 +57,12 @@ def test_argument_errors_need_no_device():
     assert lib.bfXcorrCreate(ctypes.byref(plan), 8, 1, 3, 4) == 5            # UNSUPPORTED_SHAPE (8-byte rows)
     assert lib.bfXcorrDestroy(None) == 2                                     # INVALID_HANDLE
     assert lib.bfXcorrExecute(None, None, None, 0, None) == 2
+    assert lib.bfBeamformCreate(None, 16, 4, 256, 2, 8) == 1
+    assert lib.bfBeamformCreate(ctypes.byref(plan), 16, 4, 256, 0, 8) == 3   # nbeam <= 0
+    assert lib.bfBeamformCreate(ctypes.byref(plan), 16, 4, 256, 2, 5) == 4
+    assert lib.bfBeamformCreate(ctypes.byref(plan), 16, 4, 256, 129, 8) == 5  # nbeam > 128
+    assert lib.bfBeamformCreate(ctypes.byref(plan), 8, 1, 3, 1, 4) == 5      # 8-byte rows
+    assert lib.bfBeamformExecute(None, None, None, None) == 2
 
 
 def test_no_cpu_fallback_without_a_device():
