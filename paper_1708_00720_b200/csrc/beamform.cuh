@@ -15,10 +15,12 @@
 // so the CTAs of one wave read adjacent channels of the same samples (whole DRAM pages) and a group's weights stay
 // in the L2 while its sample blocks go by.
 //
-// Roles (512 threads, one CTA per SM): warp 0 weight producer (TMA, 128B-swizzled K-major boxes), warp 1 MMA issuer,
-// warp 2 TMEM allocator, warps 4..7 epilogue (TMEM -> registers -> global, one sample row per thread), warps 8..15
-// loaders: coalesced 16-byte span loads, two stages in flight per thread, written (ci4: widened) into the
-// 128B-swizzled K-major layout the UMMA descriptor expects.
+// Roles (512 threads, one CTA per SM): warp 0 span producer (TMA boxes of 128 span bytes x 128 samples of one channel:
+// ci8 lands 128B-swizzled straight in the operand stage, ci4 lands raw in a ring), warp 3 weight producer (ci4 only; for
+// ci8 warp 0 loads both), warp 1 MMA issuer, warp 2 TMEM allocator, warps 4..7 epilogue (TMEM -> registers -> global,
+// one sample row per thread), warps 8..15 (ci4 only) widen raw rows into the 128B-swizzled K-major int8 layout the
+// UMMA descriptor expects.  TMA keeps every free stage in flight (up to 128 KB per SM), which register-staged loads
+// could not (profiles/round1.md).
 #pragma once
 #include <cstdint>
 #include <cuda.h>
@@ -30,7 +32,7 @@ constexpr int BM_MT = 128;             // samples per unit
 constexpr int BM_LOAD_WARPS = 8;
 constexpr int BM_THREADS = 256 + 32 * BM_LOAD_WARPS;
 constexpr int BM_MAX_STAGES = 8;
-constexpr int BM_DEPTH = 2;            // span stages in flight per loader thread
+constexpr int BM_MAX_RAW = 4;          // raw ci4 stages (16 KB each)
 constexpr int BM_SMEM_MAX = 232448 - 1024;
 
 struct BmParams {
@@ -42,7 +44,8 @@ struct BmParams {
     int nks;         // K stages: ceil(row_in / 128)
     int ntb;         // sample blocks: ceil(ntime / 128)
     int group;       // adjacent channels per scheduling group
-    int stages;      // pipeline depth
+    int stages;      // operand stages
+    int raw_stages;  // raw ci4 stages (0 for ci8)
     long long nunits;
 };
 
@@ -81,7 +84,7 @@ __host__ __device__ constexpr uint32_t bm_instr_desc(int m, int n)
 
 template <bool CI4>
 __global__ void __launch_bounds__(BM_THREADS, 1)
-beamform_kernel(const __grid_constant__ CUtensorMap wmap, const BmParams p)
+beamform_kernel(const __grid_constant__ CUtensorMap xmap, const __grid_constant__ CUtensorMap wmap, const BmParams p)
 {
     constexpr int KS = CI4 ? 256 : 128;        // int8 K bytes per stage (128 span bytes)
     constexpr int KH = KS / 128;               // 128-byte K tiles per stage
@@ -91,21 +94,30 @@ beamform_kernel(const __grid_constant__ CUtensorMap wmap, const BmParams p)
     const uint32_t w_tile = static_cast<uint32_t>(p.nb2) * 128u;
     const uint32_t stage_bytes = KH * (A_TILE + w_tile);
     const int S = p.stages;
-    const uint32_t bar_base = smem_base + S * stage_bytes;
+    const int R = p.raw_stages;
+    const uint32_t raw_base = smem_base + S * stage_bytes;      // [R] raw ci4 tiles [128 samples][128 bytes]
+    const uint32_t bar_base = raw_base + R * A_TILE;
     const uint32_t bar_full = bar_base;                          // [S] span tile written + weight boxes landed
     const uint32_t bar_empty = bar_full + 8 * BM_MAX_STAGES;     // [S] MMAs reading the stage have completed
     const uint32_t bar_tfull = bar_empty + 8 * BM_MAX_STAGES;    // [2] accumulator complete
     const uint32_t bar_tempty = bar_tfull + 16;                  // [2] accumulator drained
-    const uint32_t tmem_slot = bar_tempty + 16;
+    const uint32_t bar_rfull = bar_tempty + 16;                  // [R] raw bytes landed
+    const uint32_t bar_rempty = bar_rfull + 8 * BM_MAX_RAW;      // [R] raw bytes consumed by the widening warps
+    const uint32_t tmem_slot = bar_rempty + 8 * BM_MAX_RAW;
 
     const int warp = threadIdx.x >> 5;
     const uint32_t lane = ptx::lane_id();
 
     if (warp == 0 && lane == 0) {
+        ptx::prefetch_tensormap(&xmap);
         ptx::prefetch_tensormap(&wmap);
         for (int s = 0; s < S; ++s) {
-            ptx::mbar_init(bar_full + 8 * s, BM_LOAD_WARPS + 1);
+            ptx::mbar_init(bar_full + 8 * s, CI4 ? BM_LOAD_WARPS + 1 : 1);
             ptx::mbar_init(bar_empty + 8 * s, 1);
+        }
+        for (int s = 0; s < R; ++s) {
+            ptx::mbar_init(bar_rfull + 8 * s, 1);
+            ptx::mbar_init(bar_rempty + 8 * s, BM_LOAD_WARPS);
         }
         for (int b = 0; b < 2; ++b) {
             ptx::mbar_init(bar_tfull + 8 * b, 1);
@@ -126,21 +138,49 @@ beamform_kernel(const __grid_constant__ CUtensorMap wmap, const BmParams p)
     const long long u0 = blockIdx.x, ustep = gridDim.x;
 
     if (warp == 0) {
-        // ===================== weight producer (converged warp, lane 0 issues) =====================
+        // ===================== span producer (converged warp, lane 0 issues); ci8: the weights too =====================
         uint32_t stage = 0, phase = 0;
+        const uint32_t nst = CI4 ? static_cast<uint32_t>(R) : static_cast<uint32_t>(S);
         for (long long u = u0; u < p.nunits; u += ustep) {
             const BmUnit un = bm_decode(p, u);
             for (int ks = 0; ks < p.nks; ++ks) {
-                ptx::mbar_wait(bar_empty + 8 * stage, phase ^ 1);
-                if (lane == 0) {
-                    const uint32_t dst = smem_base + stage * stage_bytes + KH * A_TILE;
-                    ptx::mbar_expect_tx(bar_full + 8 * stage, KH * w_tile);
-#pragma unroll
-                    for (int h = 0; h < KH; ++h)
-                        ptx::tma_load_2d(dst + h * w_tile, &wmap, bar_full + 8 * stage, ks * KS + h * 128, un.c * p.nb2);
+                if (CI4) {
+                    ptx::mbar_wait(bar_rempty + 8 * stage, phase ^ 1);
+                    if (lane == 0) {
+                        ptx::mbar_expect_tx(bar_rfull + 8 * stage, A_TILE);
+                        ptx::tma_load_3d(raw_base + stage * A_TILE, &xmap, bar_rfull + 8 * stage, ks * 128, un.c, un.t0);
+                    }
+                } else {
+                    ptx::mbar_wait(bar_empty + 8 * stage, phase ^ 1);
+                    if (lane == 0) {
+                        const uint32_t dst = smem_base + stage * stage_bytes;
+                        ptx::mbar_expect_tx(bar_full + 8 * stage, A_TILE + w_tile);
+                        ptx::tma_load_3d(dst, &xmap, bar_full + 8 * stage, ks * 128, un.c, un.t0);
+                        ptx::tma_load_2d(dst + A_TILE, &wmap, bar_full + 8 * stage, ks * KS, un.c * p.nb2);
+                    }
                 }
                 __syncwarp();
-                if (++stage == static_cast<uint32_t>(S)) { stage = 0; phase ^= 1; }
+                if (++stage == nst) { stage = 0; phase ^= 1; }
+            }
+        }
+    } else if (warp == 3) {
+        // ===================== weight producer, ci4 (converged warp, lane 0 issues) =====================
+        if (CI4) {
+            uint32_t stage = 0, phase = 0;
+            for (long long u = u0; u < p.nunits; u += ustep) {
+                const BmUnit un = bm_decode(p, u);
+                for (int ks = 0; ks < p.nks; ++ks) {
+                    ptx::mbar_wait(bar_empty + 8 * stage, phase ^ 1);
+                    if (lane == 0) {
+                        const uint32_t dst = smem_base + stage * stage_bytes + KH * A_TILE;
+                        ptx::mbar_expect_tx(bar_full + 8 * stage, KH * w_tile);
+#pragma unroll
+                        for (int h = 0; h < KH; ++h)
+                            ptx::tma_load_2d(dst + h * w_tile, &wmap, bar_full + 8 * stage, ks * KS + h * 128, un.c * p.nb2);
+                    }
+                    __syncwarp();
+                    if (++stage == static_cast<uint32_t>(S)) { stage = 0; phase ^= 1; }
+                }
             }
         }
     } else if (warp == 1) {
@@ -193,7 +233,11 @@ beamform_kernel(const __grid_constant__ CUtensorMap wmap, const BmParams p)
 #pragma unroll
                     for (int j = 0; j < 32; ++j) r[j] = static_cast<uint32_t>(static_cast<int32_t>(r[j]) >> 4);
                 }
+#ifdef BFX_BM_NO_STORE
+                if (t < -p.ntime) {
+#else
                 if (t < p.ntime) {
+#endif
                     if (vec4) {
 #pragma unroll
                         for (int j = 0; j < 32; j += 4)
@@ -212,83 +256,44 @@ beamform_kernel(const __grid_constant__ CUtensorMap wmap, const BmParams p)
             if (lane == 0) ptx::mbar_arrive(bar_tempty + 8 * b);
         }
     } else if (warp >= 8) {
-        // ===================== loaders: span rows -> swizzled K-major int8 tiles =====================
-        // vector v = i * 256 + tid of a stage: sample row v >> 3, 16-byte chunk v & 7 of the row's 128 span bytes;
-        // eight lanes read one whole 128-byte line and (ci8) write one whole swizzled row
-        const int tid = static_cast<int>(threadIdx.x) - 256;
-        const int chunk = tid & 7;
-        struct It {
-            long long u;
-            int ks, c, t0;
-        };
-        It li{u0, 0, 0, 0}, si{u0, 0, 0, 0};
-        if (u0 < p.nunits) {
-            const BmUnit un = bm_decode(p, u0);
-            li.c = si.c = un.c;
-            li.t0 = si.t0 = un.t0;
-        }
-        auto advance = [&](It& a) {
-            if (++a.ks == p.nks) {
-                a.ks = 0;
-                a.u += ustep;
-                if (a.u < p.nunits) {
-                    const BmUnit un = bm_decode(p, a.u);
-                    a.c = un.c;
-                    a.t0 = un.t0;
-                }
-            }
-        };
-        uint4 buf[BM_DEPTH][4];
-        auto issue = [&](const It& a, uint4* v) {
-            const int kbyte = a.ks * 128 + chunk * 16;
-#pragma unroll
-            for (int i = 0; i < 4; ++i) {
-                const int t = a.t0 + i * 32 + (tid >> 3);
-                v[i] = make_uint4(0u, 0u, 0u, 0u);
-                if (a.u < p.nunits && t < p.ntime && kbyte < p.row_in)
-                    v[i] = ptx::ld_global_stream_v4(p.x + (static_cast<long long>(t) * p.nchan + a.c) * p.row_in + kbyte);
-            }
-        };
-#pragma unroll
-        for (int d = 0; d < BM_DEPTH; ++d) {
-            issue(li, buf[d]);
-            advance(li);
-        }
-        uint32_t stage = 0, phase = 0;
-        while (si.u < p.nunits) {
-#pragma unroll
-            for (int d = 0; d < BM_DEPTH; ++d) {
-                if (si.u < p.nunits) {
+        // ===================== ci4: raw rows -> swizzled K-major int8 tiles =====================
+        // vector v = i * 256 + tid of a stage: sample row v >> 3, 16-byte chunk v & 7 of the row's 128 raw bytes (16
+        // samples), widened to chunks 2 * chunk and 2 * chunk + 1 of the row's 256 int8 bytes
+        if (CI4) {
+            const int tid = static_cast<int>(threadIdx.x) - 256;
+            const int chunk = tid & 7;
+            uint32_t rstage = 0, rphase = 0, stage = 0, phase = 0;
+            for (long long u = u0; u < p.nunits; u += ustep) {
+                for (int ks = 0; ks < p.nks; ++ks) {
+                    ptx::mbar_wait(bar_rfull + 8 * rstage, rphase);
                     ptx::mbar_wait(bar_empty + 8 * stage, phase ^ 1);
+                    const uint32_t rsrc = raw_base + rstage * A_TILE;
                     const uint32_t abase = smem_base + stage * stage_bytes;
 #pragma unroll
                     for (int i = 0; i < 4; ++i) {
                         const int rowi = i * 32 + (tid >> 3);
-                        const uint4 w = buf[d][i];
-                        const uint32_t rowa = abase + rowi * 128;
-                        if (CI4) {
-                            // 16 packed samples -> chunks 2 * chunk and 2 * chunk + 1 of the 256-byte int8 row
-                            const uint32_t tile = rowa + (chunk >> 2) * A_TILE;
-                            const uint32_t j0 = static_cast<uint32_t>(2 * chunk) & 7u;
-                            const uint32_t a0 = tile + ((j0 ^ (rowi & 7)) << 4), a1 = tile + (((j0 + 1) ^ (rowi & 7)) << 4);
-                            asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(a0), "r"(w.x & 0xF0F0F0F0u),
-                                         "r"((w.x << 4) & 0xF0F0F0F0u), "r"(w.y & 0xF0F0F0F0u), "r"((w.y << 4) & 0xF0F0F0F0u)
-                                         : "memory");
-                            asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(a1), "r"(w.z & 0xF0F0F0F0u),
-                                         "r"((w.z << 4) & 0xF0F0F0F0u), "r"(w.w & 0xF0F0F0F0u), "r"((w.w << 4) & 0xF0F0F0F0u)
-                                         : "memory");
-                        } else {
-                            const uint32_t a0 = rowa + ((static_cast<uint32_t>(chunk) ^ (rowi & 7)) << 4);
-                            asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(a0), "r"(w.x), "r"(w.y), "r"(w.z), "r"(w.w) : "memory");
-                        }
+                        uint4 w;
+                        asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
+                                     : "=r"(w.x), "=r"(w.y), "=r"(w.z), "=r"(w.w)
+                                     : "r"(rsrc + rowi * 128 + chunk * 16));
+                        const uint32_t tile = abase + rowi * 128 + (chunk >> 2) * A_TILE;
+                        const uint32_t j0 = static_cast<uint32_t>(2 * chunk) & 7u;
+                        const uint32_t a0 = tile + ((j0 ^ (rowi & 7)) << 4), a1 = tile + (((j0 + 1) ^ (rowi & 7)) << 4);
+                        asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(a0), "r"(w.x & 0xF0F0F0F0u),
+                                     "r"((w.x << 4) & 0xF0F0F0F0u), "r"(w.y & 0xF0F0F0F0u), "r"((w.y << 4) & 0xF0F0F0F0u)
+                                     : "memory");
+                        asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(a1), "r"(w.z & 0xF0F0F0F0u),
+                                     "r"((w.z << 4) & 0xF0F0F0F0u), "r"(w.w & 0xF0F0F0F0u), "r"((w.w << 4) & 0xF0F0F0F0u)
+                                     : "memory");
                     }
                     ptx::fence_proxy_async_smem();  // generic-proxy stores -> visible to the tensor core (async proxy)
                     __syncwarp();
-                    if (lane == 0) ptx::mbar_arrive(bar_full + 8 * stage);
+                    if (lane == 0) {
+                        ptx::mbar_arrive(bar_rempty + 8 * rstage);
+                        ptx::mbar_arrive(bar_full + 8 * stage);
+                    }
+                    if (++rstage == static_cast<uint32_t>(R)) { rstage = 0; rphase ^= 1; }
                     if (++stage == static_cast<uint32_t>(S)) { stage = 0; phase ^= 1; }
-                    issue(li, buf[d]);
-                    advance(li);
-                    advance(si);
                 }
             }
         }

@@ -30,6 +30,7 @@ struct bfBeamform_impl {
     int* d_bad;     // set by the re-ordering kernel if an imaginary part is -128
     int nb2, kp;
     CUtensorMap wmap;
+    EncodeTiledFn encode;
     bfx::BmParams prm;
     unsigned smem_bytes;
 };
@@ -113,10 +114,15 @@ int bfBeamformCreate(bfBeamform* plan, int ninputs, int nchan, int ntime, int nb
     p->nb2 = q.nb2;
     p->kp = q.nks * ks_bytes;
     const unsigned stage_bytes = static_cast<unsigned>(ks_bytes / 128) * (bfx::BM_MT * 128u + static_cast<unsigned>(q.nb2) * 128u);
-    int stages = static_cast<int>((bfx::BM_SMEM_MAX - 1536) / stage_bytes);
+    // ci4: raw ring of 16 KB tiles beside the operand stages (2 when the stages are at their largest, else 4)
+    const unsigned raw_tile = bfx::BM_MT * 128u;
+    int raw = ci4 ? (2u * stage_bytes + 4u * raw_tile + 1536u <= static_cast<unsigned>(bfx::BM_SMEM_MAX) ? 4 : 2) : 0;
+    int stages = static_cast<int>((bfx::BM_SMEM_MAX - 1536 - raw * raw_tile) / stage_bytes);
     if (stages > bfx::BM_MAX_STAGES) stages = bfx::BM_MAX_STAGES;
     q.stages = stages;  // >= 2 for every nb2 <= 256
-    p->smem_bytes = 1024u + static_cast<unsigned>(stages) * stage_bytes + 512u;
+    q.raw_stages = raw;
+    p->smem_bytes = 1024u + static_cast<unsigned>(stages) * stage_bytes + raw * raw_tile + 512u;
+    p->encode = reinterpret_cast<EncodeTiledFn>(fn);
     // a group's weights (group * nb2 * kp bytes) should stay in the L2 while its sample blocks go by
     long long group = (32ll << 20) / (static_cast<long long>(q.nb2) * p->kp);
     if (group < 1) group = 1;
@@ -190,10 +196,24 @@ int bfBeamformExecute(bfBeamform p, const void* in, void* out, void* stream)
     q.out = static_cast<int32_t*>(out);
     const unsigned grid = static_cast<unsigned>(q.nunits < p->num_sms ? q.nunits : p->num_sms);
     cudaStream_t s = static_cast<cudaStream_t>(stream);
-    if (p->dtype == BF_XCORR_CI4)
-        bfx::beamform_kernel<true><<<grid, bfx::BM_THREADS, p->smem_bytes, s>>>(p->wmap, q);
+    // span boxes: 128 bytes of a row x 1 channel x 128 samples; rows and samples beyond the span read as zeros
+    const bool ci4 = p->dtype == BF_XCORR_CI4;
+    CUtensorMap xmap;
+    const cuuint64_t dims[3] = {static_cast<cuuint64_t>(q.row_in), static_cast<cuuint64_t>(p->nchan), static_cast<cuuint64_t>(p->ntime)};
+    const cuuint64_t strides[2] = {static_cast<cuuint64_t>(q.row_in), static_cast<cuuint64_t>(q.row_in) * p->nchan};
+    const cuuint32_t box[3] = {128u, 1u, static_cast<cuuint32_t>(bfx::BM_MT)};
+    const cuuint32_t estr[3] = {1u, 1u, 1u};
+    const CUresult r = p->encode(&xmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<void*>(in), dims, strides, box, estr,
+                                 CU_TENSOR_MAP_INTERLEAVE_NONE, ci4 ? CU_TENSOR_MAP_SWIZZLE_NONE : CU_TENSOR_MAP_SWIZZLE_128B,
+                                 CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        p->last_cuda_error = static_cast<int>(cudaErrorInvalidValue);
+        return BF_XCORR_DEVICE_ERROR;
+    }
+    if (ci4)
+        bfx::beamform_kernel<true><<<grid, bfx::BM_THREADS, p->smem_bytes, s>>>(xmap, p->wmap, q);
     else
-        bfx::beamform_kernel<false><<<grid, bfx::BM_THREADS, p->smem_bytes, s>>>(p->wmap, q);
+        bfx::beamform_kernel<false><<<grid, bfx::BM_THREADS, p->smem_bytes, s>>>(xmap, p->wmap, q);
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(p, e);
     return BF_XCORR_OK;
