@@ -17,8 +17,8 @@
 //
 // Roles (512 threads, one CTA per SM): warp 0 span producer (TMA boxes of 128 span bytes x 128 samples of one channel:
 // ci8 lands 128B-swizzled straight in the operand stage, ci4 lands raw in a ring), warp 3 weight producer (ci4 only; for
-// ci8 warp 0 loads both), warp 1 MMA issuer, warp 2 TMEM allocator, warps 4..7 epilogue (TMEM -> registers -> global,
-// one sample row per thread), warps 8..15 (ci4 only) widen raw rows into the 128B-swizzled K-major int8 layout the
+// ci8 warp 0 loads both), warp 1 MMA issuer, warp 2 TMEM allocator, warps 4..7 epilogue (TMEM -> registers -> shared
+// staging -> global, eight lanes per 128-byte row piece), warps 8..15 (ci4 only) widen raw rows into the 128B-swizzled K-major int8 layout the
 // UMMA descriptor expects.  TMA keeps every free stage in flight (up to 128 KB per SM), which register-staged loads
 // could not (profiles/round1.md).
 #pragma once
@@ -33,6 +33,9 @@ constexpr int BM_LOAD_WARPS = 8;
 constexpr int BM_THREADS = 256 + 32 * BM_LOAD_WARPS;
 constexpr int BM_MAX_STAGES = 8;
 constexpr int BM_MAX_RAW = 4;          // raw ci4 stages (16 KB each)
+constexpr int BM_STG_PITCH = 144;      // epilogue staging: 32 rows x 128 bytes, pitch 144 -> conflict-free 16-byte accesses
+constexpr int BM_STG_WARP = 32 * BM_STG_PITCH;
+constexpr int BM_STG_BYTES = 4 * BM_STG_WARP;
 constexpr int BM_SMEM_MAX = 232448 - 1024;
 
 struct BmParams {
@@ -96,7 +99,8 @@ beamform_kernel(const __grid_constant__ CUtensorMap xmap, const __grid_constant_
     const int S = p.stages;
     const int R = p.raw_stages;
     const uint32_t raw_base = smem_base + S * stage_bytes;      // [R] raw ci4 tiles [128 samples][128 bytes]
-    const uint32_t bar_base = raw_base + R * A_TILE;
+    const uint32_t stg_base = raw_base + R * A_TILE;            // epilogue staging, one buffer per warp
+    const uint32_t bar_base = stg_base + BM_STG_BYTES;
     const uint32_t bar_full = bar_base;                          // [S] span tile written + weight boxes landed
     const uint32_t bar_empty = bar_full + 8 * BM_MAX_STAGES;     // [S] MMAs reading the stage have completed
     const uint32_t bar_tfull = bar_empty + 8 * BM_MAX_STAGES;    // [2] accumulator complete
@@ -139,6 +143,8 @@ beamform_kernel(const __grid_constant__ CUtensorMap xmap, const __grid_constant_
 
     if (warp == 0) {
         // ===================== span producer (converged warp, lane 0 issues); ci8: the weights too =====================
+        // the span is read once (evict first); a group's weights are re-read by every sample block (evict last)
+        const uint64_t pol_first = ptx::policy_evict_first(), pol_last = ptx::policy_evict_last();
         uint32_t stage = 0, phase = 0;
         const uint32_t nst = CI4 ? static_cast<uint32_t>(R) : static_cast<uint32_t>(S);
         for (long long u = u0; u < p.nunits; u += ustep) {
@@ -148,15 +154,15 @@ beamform_kernel(const __grid_constant__ CUtensorMap xmap, const __grid_constant_
                     ptx::mbar_wait(bar_rempty + 8 * stage, phase ^ 1);
                     if (lane == 0) {
                         ptx::mbar_expect_tx(bar_rfull + 8 * stage, A_TILE);
-                        ptx::tma_load_3d(raw_base + stage * A_TILE, &xmap, bar_rfull + 8 * stage, ks * 128, un.c, un.t0);
+                        ptx::tma_load_3d_hint(raw_base + stage * A_TILE, &xmap, bar_rfull + 8 * stage, ks * 128, un.c, un.t0, pol_first);
                     }
                 } else {
                     ptx::mbar_wait(bar_empty + 8 * stage, phase ^ 1);
                     if (lane == 0) {
                         const uint32_t dst = smem_base + stage * stage_bytes;
                         ptx::mbar_expect_tx(bar_full + 8 * stage, A_TILE + w_tile);
-                        ptx::tma_load_3d(dst, &xmap, bar_full + 8 * stage, ks * 128, un.c, un.t0);
-                        ptx::tma_load_2d(dst + A_TILE, &wmap, bar_full + 8 * stage, ks * KS, un.c * p.nb2);
+                        ptx::tma_load_3d_hint(dst, &xmap, bar_full + 8 * stage, ks * 128, un.c, un.t0, pol_first);
+                        ptx::tma_load_2d_hint(dst + A_TILE, &wmap, bar_full + 8 * stage, ks * KS, un.c * p.nb2, pol_last);
                     }
                 }
                 __syncwarp();
@@ -166,6 +172,7 @@ beamform_kernel(const __grid_constant__ CUtensorMap xmap, const __grid_constant_
     } else if (warp == 3) {
         // ===================== weight producer, ci4 (converged warp, lane 0 issues) =====================
         if (CI4) {
+            const uint64_t pol_last = ptx::policy_evict_last();
             uint32_t stage = 0, phase = 0;
             for (long long u = u0; u < p.nunits; u += ustep) {
                 const BmUnit un = bm_decode(p, u);
@@ -176,7 +183,7 @@ beamform_kernel(const __grid_constant__ CUtensorMap xmap, const __grid_constant_
                         ptx::mbar_expect_tx(bar_full + 8 * stage, KH * w_tile);
 #pragma unroll
                         for (int h = 0; h < KH; ++h)
-                            ptx::tma_load_2d(dst + h * w_tile, &wmap, bar_full + 8 * stage, ks * KS + h * 128, un.c * p.nb2);
+                            ptx::tma_load_2d_hint(dst + h * w_tile, &wmap, bar_full + 8 * stage, ks * KS + h * 128, un.c * p.nb2, pol_last);
                     }
                     __syncwarp();
                     if (++stage == static_cast<uint32_t>(S)) { stage = 0; phase ^= 1; }
@@ -218,6 +225,7 @@ beamform_kernel(const __grid_constant__ CUtensorMap xmap, const __grid_constant_
         const int wq = warp - 4;
         uint32_t it = 0;
         const bool vec4 = (p.nbeam & 1) == 0;
+        const uint32_t stg_warp = stg_base + wq * BM_STG_WARP;
         for (long long u = u0; u < p.nunits; u += ustep, ++it) {
             const BmUnit un = bm_decode(p, u);
             const uint32_t b = it & 1;
@@ -225,6 +233,7 @@ beamform_kernel(const __grid_constant__ CUtensorMap xmap, const __grid_constant_
             ptx::tc_fence_after();
             const int t = un.t0 + 32 * wq + static_cast<int>(lane);
             int32_t* const orow = p.out + 2 * ((static_cast<long long>(t) * p.nchan + un.c) * p.nbeam);
+            const int nrows = p.ntime - (un.t0 + 32 * wq);   // rows of this warp that exist
             for (int col = 0; col < 2 * p.nbeam; col += 32) {
                 uint32_t r[32];
                 ptx::tmem_ld_32x32b_x32(tmem_base + (static_cast<uint32_t>(32 * wq) << 16) + 256 * b + col, r);
@@ -234,16 +243,35 @@ beamform_kernel(const __grid_constant__ CUtensorMap xmap, const __grid_constant_
                     for (int j = 0; j < 32; ++j) r[j] = static_cast<uint32_t>(static_cast<int32_t>(r[j]) >> 4);
                 }
 #ifdef BFX_BM_NO_STORE
-                if (t < -p.ntime) {
+                if (nrows < -p.ntime) {
 #else
-                if (t < p.ntime) {
+                {
 #endif
                     if (vec4) {
+                        // through shared memory so that eight lanes write one row's 128 contiguous bytes
+                        const uint32_t srow = stg_warp + lane * BM_STG_PITCH;
 #pragma unroll
                         for (int j = 0; j < 32; j += 4)
-                            if (col + j < 2 * p.nbeam)
-                                ptx::st_global_v4(reinterpret_cast<uint8_t*>(orow + col + j), make_uint4(r[j], r[j + 1], r[j + 2], r[j + 3]));
-                    } else {
+                            asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(srow + 4 * j), "r"(r[j]), "r"(r[j + 1]),
+                                         "r"(r[j + 2]), "r"(r[j + 3])
+                                         : "memory");
+                        __syncwarp();
+                        const int piece = static_cast<int>(lane) & 7, npiece = (2 * p.nbeam - col + 3) >> 2;
+                        int32_t* const obase = p.out + 2 * ((static_cast<long long>(un.t0 + 32 * wq) * p.nchan + un.c) * p.nbeam) + col + 4 * piece;
+                        const long long rstride = 2ll * p.nchan * p.nbeam;
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) {
+                            const int row = 4 * i + (static_cast<int>(lane) >> 3);
+                            if (row < nrows && piece < npiece) {
+                                uint4 v;
+                                asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
+                                             : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w)
+                                             : "r"(stg_warp + row * BM_STG_PITCH + piece * 16));
+                                ptx::st_global_v4(reinterpret_cast<uint8_t*>(obase + row * rstride), v);
+                            }
+                        }
+                        __syncwarp();
+                    } else if (static_cast<int>(lane) < nrows) {
 #pragma unroll
                         for (int j = 0; j < 32; j += 2)
                             if (col + j < 2 * p.nbeam)
@@ -279,11 +307,16 @@ beamform_kernel(const __grid_constant__ CUtensorMap xmap, const __grid_constant_
                         const uint32_t tile = abase + rowi * 128 + (chunk >> 2) * A_TILE;
                         const uint32_t j0 = static_cast<uint32_t>(2 * chunk) & 7u;
                         const uint32_t a0 = tile + ((j0 ^ (rowi & 7)) << 4), a1 = tile + (((j0 + 1) ^ (rowi & 7)) << 4);
-                        asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(a0), "r"(w.x & 0xF0F0F0F0u),
-                                     "r"((w.x << 4) & 0xF0F0F0F0u), "r"(w.y & 0xF0F0F0F0u), "r"((w.y << 4) & 0xF0F0F0F0u)
+                        // chunks c and c + 4 of a row fall on the same banks (different K tiles): the upper four lanes of
+                        // a row write their odd chunk first, so every store covers all 32 banks once
+                        const bool hi = (chunk & 4) != 0;
+                        const uint32_t e0 = w.x & 0xF0F0F0F0u, e1 = (w.x << 4) & 0xF0F0F0F0u, e2 = w.y & 0xF0F0F0F0u, e3 = (w.y << 4) & 0xF0F0F0F0u;
+                        const uint32_t o0 = w.z & 0xF0F0F0F0u, o1 = (w.z << 4) & 0xF0F0F0F0u, o2 = w.w & 0xF0F0F0F0u, o3 = (w.w << 4) & 0xF0F0F0F0u;
+                        asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(hi ? a1 : a0), "r"(hi ? o0 : e0), "r"(hi ? o1 : e1),
+                                     "r"(hi ? o2 : e2), "r"(hi ? o3 : e3)
                                      : "memory");
-                        asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(a1), "r"(w.z & 0xF0F0F0F0u),
-                                     "r"((w.z << 4) & 0xF0F0F0F0u), "r"(w.w & 0xF0F0F0F0u), "r"((w.w << 4) & 0xF0F0F0F0u)
+                        asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(hi ? a0 : a1), "r"(hi ? e0 : o0), "r"(hi ? e1 : o1),
+                                     "r"(hi ? e2 : o2), "r"(hi ? e3 : o3)
                                      : "memory");
                     }
                     ptx::fence_proxy_async_smem();  // generic-proxy stores -> visible to the tensor core (async proxy)

@@ -16,6 +16,13 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
+#ifndef BFX_BM_GROUP_MB
+#define BFX_BM_GROUP_MB 8
+#endif
+#ifndef BFX_BM_PROMO
+#define BFX_BM_PROMO CU_TENSOR_MAP_L2_PROMOTION_L2_256B
+#endif
+
 constexpr uint32_t kMagic = 0xBFBEA301u;
 
 }  // namespace
@@ -116,15 +123,16 @@ int bfBeamformCreate(bfBeamform* plan, int ninputs, int nchan, int ntime, int nb
     const unsigned stage_bytes = static_cast<unsigned>(ks_bytes / 128) * (bfx::BM_MT * 128u + static_cast<unsigned>(q.nb2) * 128u);
     // ci4: raw ring of 16 KB tiles beside the operand stages (2 when the stages are at their largest, else 4)
     const unsigned raw_tile = bfx::BM_MT * 128u;
-    int raw = ci4 ? (2u * stage_bytes + 4u * raw_tile + 1536u <= static_cast<unsigned>(bfx::BM_SMEM_MAX) ? 4 : 2) : 0;
-    int stages = static_cast<int>((bfx::BM_SMEM_MAX - 1536 - raw * raw_tile) / stage_bytes);
+    const unsigned fixed = 1536u + bfx::BM_STG_BYTES;
+    int raw = ci4 ? (2u * stage_bytes + 4u * raw_tile + fixed <= static_cast<unsigned>(bfx::BM_SMEM_MAX) ? 4 : 2) : 0;
+    int stages = static_cast<int>((bfx::BM_SMEM_MAX - fixed - raw * raw_tile) / stage_bytes);
     if (stages > bfx::BM_MAX_STAGES) stages = bfx::BM_MAX_STAGES;
     q.stages = stages;  // >= 2 for every nb2 <= 256
     q.raw_stages = raw;
-    p->smem_bytes = 1024u + static_cast<unsigned>(stages) * stage_bytes + raw * raw_tile + 512u;
+    p->smem_bytes = static_cast<unsigned>(stages) * stage_bytes + raw * raw_tile + fixed;
     p->encode = reinterpret_cast<EncodeTiledFn>(fn);
-    // a group's weights (group * nb2 * kp bytes) should stay in the L2 while its sample blocks go by
-    long long group = (32ll << 20) / (static_cast<long long>(q.nb2) * p->kp);
+    // a group's weights (group * nb2 * kp bytes, about 8 MB) stay in the L2 (evict-last loads) while its sample blocks go by
+    long long group = (static_cast<long long>(BFX_BM_GROUP_MB) << 20) / (static_cast<long long>(q.nb2) * p->kp);
     if (group < 1) group = 1;
     if (group > nchan) group = nchan;
     q.group = static_cast<int>(group);
@@ -205,7 +213,7 @@ int bfBeamformExecute(bfBeamform p, const void* in, void* out, void* stream)
     const cuuint32_t estr[3] = {1u, 1u, 1u};
     const CUresult r = p->encode(&xmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<void*>(in), dims, strides, box, estr,
                                  CU_TENSOR_MAP_INTERLEAVE_NONE, ci4 ? CU_TENSOR_MAP_SWIZZLE_NONE : CU_TENSOR_MAP_SWIZZLE_128B,
-                                 CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                                 BFX_BM_PROMO, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) {
         p->last_cuda_error = static_cast<int>(cudaErrorInvalidValue);
         return BF_XCORR_DEVICE_ERROR;
