@@ -189,6 +189,90 @@ def run_reference(args, cfg):
     print(json.dumps(line), flush=True)
 
 
+def run_beamform(args, cfg):
+    """Second workload on the same spans (include/bfbeamform.h): one step = every span of the config beamformed once."""
+    import numpy as np
+    import torch
+    import oracle
+    import paper_1708_00720_b200 as bfx
+    from xcorr_inputs import generate_channel_slab, generate_span, generate_weights
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the beamformer has no CPU fallback")
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    K, N, C, T = args.nbeam, cfg.ninputs, cfg.nchan, cfg.ntime
+    peaks = load_peaks()
+    spans = [generate_span(cfg, s, device=dev) for s in range(cfg.nspans)]
+    w = generate_weights(cfg.seed, C, K, N, device=dev)
+    out = torch.empty((T, C, K, 2), dtype=torch.int32, device=dev)
+    plan = bfx.bfBeamformCreate(N, C, T, K, cfg.dtype)
+    stream = torch.cuda.current_stream()
+    bfx.bfBeamformSetWeights(plan, w.data_ptr(), stream.cuda_stream)
+    flush = None if cfg.span_bytes * cfg.nspans > 126e6 else torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+
+    def step(rec=None):
+        for s in range(cfg.nspans):
+            if flush is not None:
+                flush.zero_()
+            e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            bfx.bfBeamformExecute(plan, spans[s].data_ptr(), out.data_ptr(), stream.cuda_stream)
+            e1.record(stream)
+            if rec is not None:
+                rec.append((e0, e1))
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(0)
+    sampler.start()
+    rec = []
+    for _ in range(args.steps):
+        step(rec)
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    launch_ms = [a.elapsed_time(b) for a, b in rec]
+    t_launch = sum(launch_ms) / len(launch_ms) * 1e-3
+    ms_per_step = t_launch * 1e3 * cfg.nspans       # kernel time only: an L2 flush (if any) sits between launches
+    bfx.bfBeamformDestroy(plan)
+    bytes_launch = float(cfg.span_bytes) + float(out.numel() * 4) + 4.0 * C * K * N   # span + beams + int8 weight rows, once each
+    samples = float(T) * C * N
+    roofline = {"bound": "hbm", "achieved": bytes_launch / t_launch / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                "traffic": None, "kernel": "beamform_kernel", "algorithmic_bytes_per_launch": bytes_launch,
+                "peak_source": peaks["source"]}
+    roofline["frac"] = roofline["achieved"] / roofline["peak"]
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            tr = json.load(f).get("beamform_%s_k%d" % (cfg.name, K))
+        if tr:
+            roofline["traffic"] = tr["dram_bytes_per_launch"]
+            roofline["traffic_source"] = tr["source"]
+    except (OSError, ValueError, KeyError):
+        pass
+    cpu = None
+    if not args.no_cpu_baseline:
+        nthreads = oracle.threads()
+        per_chan_macs = float(T) * K * N
+        nch = int(max(1, min(C, args.cpu_seconds * 2.0e8 * nthreads / per_chan_macs)))   # ~2e8 complex MAC/s/thread
+        chans = sorted(set(int(round(k * (C - 1) / max(1, nch - 1))) for k in range(nch))) if nch > 1 else [0]
+        xs = generate_channel_slab(cfg, 0, chans).numpy()
+        ws = generate_weights(cfg.seed, C, K, N, channels=chans).numpy()
+        t0 = time.perf_counter()
+        oracle.beamform(xs, ws, N, len(chans), T, K, cfg.dtype)
+        dt = time.perf_counter() - t0
+        cpu = {"value": samples * len(chans) / C / dt, "unit": "complex samples/s", "cores": nthreads, "kind": "oracle",
+               "sample": "%d of %d channels (evenly spaced), one span, all samples and beams; %.1f s" % (len(chans), C, dt)}
+    line = {"metric": "beamformer input rate (complex samples/s, %d beams)" % K, "value": samples / t_launch,
+            "unit": "complex samples/s", "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3),
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "int8 x int8 -> int32", "data": "synthetic",
+            "config": config_dict(cfg, {"op": "beamform", "nbeam": K,
+                                        "l2": "inputs_exceed_l2" if flush is None else "l2_flushed_between_launches"}),
+            "tops": 8.0 * samples * K / t_launch / 1e12, "clocks": clocks, "e2e": None,
+            "gpu_launches": len(rec), "roofline": roofline, "cpu_baseline": cpu}
+    print(json.dumps(line), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -201,11 +285,18 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--op", default="xcorr", choices=["xcorr", "beamform"],
+                    help="xcorr: the hot path (the driver's line); beamform: the second workload on the same spans "
+                         "(SURVEY.md 8f N1), 1 GPU, its own JSON line")
+    ap.add_argument("--nbeam", type=int, default=32)
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
 
     from xcorr_inputs import CONFIGS, generate_span
     cfg = CONFIGS[args.config]
+    if args.op == "beamform":
+        run_beamform(args, cfg)
+        return
     if args.impl == "reference":
         run_reference(args, cfg)
         return
