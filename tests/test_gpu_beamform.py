@@ -99,7 +99,7 @@ def test_weight_domain_is_checked():
         bfx.bfBeamformDestroy(plan)
 
 
-@pytest.mark.parametrize("name,nbeam", [("cfg2", 32), ("cfg3", 16)])
+@pytest.mark.parametrize("name,nbeam", [("cfg2", 32), ("cfg3", 16), ("cfg4", 16), ("cfg5", 8), ("cfg2", 128), ("cfg2", 7)])
 def test_full_config_sampled_channels(name, nbeam):
     """BASELINE.json's station-shaped spans at full size, in the launch configuration bench.py times: sampled
     channels (all samples, all beams) against the oracle."""

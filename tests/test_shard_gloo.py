@@ -51,9 +51,17 @@ def _worker(rank, world, port, N, C, T, seed, q):
         dist.all_reduce(full, op=dist.ReduceOp.SUM)
         t = torch.tensor([10.0 + rank], dtype=torch.float64)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        # the beamformer shards the same way: span channels and the weight rows of those channels
+        K = 3
+        w = rng.integers(-127, 128, size=(C, K, 2 * N)).astype(np.int8).view(np.uint8)
+        bmine = oracle.beamform(np.ascontiguousarray(x[:, c0:c1]), np.ascontiguousarray(w[c0:c1]), N, c1 - c0, T, K, 8)
+        bfull = torch.zeros((T, C, K, 2), dtype=torch.int32)
+        bfull[:, c0:c1] = torch.from_numpy(bmine)
+        dist.all_reduce(bfull, op=dist.ReduceOp.SUM)
         if rank == 0:
             ref = oracle.xcorr(x, N, C, T, 8)
-            q.put((bool(np.array_equal(full.numpy(), ref)), float(t.item())))
+            bref = oracle.beamform(x, w, N, C, T, K, 8)
+            q.put((bool(np.array_equal(full.numpy(), ref)) and bool(np.array_equal(bfull.numpy(), bref)), float(t.item())))
     finally:
         dist.destroy_process_group()
 
