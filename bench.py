@@ -449,7 +449,8 @@ def main():
         peaks["source"], "MEASURED_PEAKS.json" if peaks["source"] == "measured" else "B200_PROFILING.md fallback",
         "sustained" if long_region else "burst")
     roofline["kernel"] = ("xcorr_simt_kernel" if args.algo != "tcgen05" else
-                          ("xcorr_pair4_kernel" if cfg.dtype == 4 else "xcorr_pair_kernel") if cfg.ninputs > 64
+                          ("xcorr_pair4_kernel" if cfg.dtype == 4 else
+                           "xcorr_stripe_kernel" if cfg.ntime <= 1024 else "xcorr_pair_kernel") if cfg.ninputs > 64
                           else "xcorr_few_kernel")
     # context: tcgen05.mma kind::i8 issue-rate probe on this pool (profiles/round1.md): 8192 MAC/clk/SM -> 4.6 POPS at 1.9 GHz
     roofline["int8_mma_probe_peak_tops"] = 4610.0

@@ -14,6 +14,7 @@
 #include "xcorr_few.cuh"
 #include "xcorr_pair.cuh"
 #include "xcorr_pair4.cuh"
+#include "xcorr_stripe.cuh"
 #include "xcorr_common.cuh"
 
 namespace {
@@ -25,6 +26,16 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
 constexpr uint32_t kMagic = 0xBFC0DE01u;
+
+#ifndef BFX_STRIPE
+#define BFX_STRIPE 1
+#endif
+#ifndef BFX_DIRECT_MAX_BLK
+#define BFX_DIRECT_MAX_BLK 8
+#endif
+#ifndef BFX_ST_AHEAD_MB
+#define BFX_ST_AHEAD_MB 16
+#endif
 
 }  // namespace
 
@@ -38,6 +49,7 @@ struct bfXcorr_impl {
     int last_launch_count;
     // S2: lower-triangle tile table (device copy) for the tcgen05 kernel
     bool pair;            // ninputs > 64: CTA-pair kernel with fused S1; else the few-input kernel
+    bool stripe;          // ci8 pair spans of <= 1024 samples: resident-A stripes (xcorr_stripe.cuh)
     int tiles_per_chan;
     unsigned long long* d_sched;  // dynamic tile scheduler state, re-armed by the kernel itself
     EncodeTiledFn encode;
@@ -148,6 +160,7 @@ int launch_tcgen05(bfXcorr p, const void* in, void* out, int accumulate, cudaStr
     prm.ntiles = static_cast<long long>(p->tiles_per_chan) * p->nchan;
     prm.accumulate = accumulate ? 1 : 0;
     prm.sched = p->d_sched;
+    prm.ring_w = p->nchan;   // no ring: the operand source is the span itself
     if (fused) {
         // ci4 spans keep their bytes in the ring (xcorr_pair4.cuh widens them in shared memory)
         prm.rl_row_out = static_cast<int>(ring_row_bytes(p));
@@ -169,13 +182,15 @@ int launch_tcgen05(bfXcorr p, const void* in, void* out, int accumulate, cudaStr
     cudaError_t e = cudaSuccess;
     if (pair) {
         // one cluster of two CTAs per tile in flight
+        const bool stripe = p->stripe && !pair4;
+        if (stripe) prm.ntiles = static_cast<long long>(p->nchan) * ((p->ninputs + bfx::PR_BLK - 1) / bfx::PR_BLK);  // stripes
         long long pairs = p->num_sms / 2;
         if (prm.ntiles < pairs) pairs = prm.ntiles;
         cudaLaunchConfig_t cfg;
         std::memset(&cfg, 0, sizeof(cfg));
         cfg.gridDim = dim3(static_cast<unsigned>(2 * pairs));
         cfg.blockDim = dim3(pair4 ? bfx::P4_THREADS : bfx::PR_THREADS);
-        cfg.dynamicSmemBytes = pair4 ? bfx::P4_SMEM_BYTES : bfx::PR_SMEM_BYTES;
+        cfg.dynamicSmemBytes = pair4 ? bfx::P4_SMEM_BYTES : stripe ? bfx::ST_SMEM_BYTES : bfx::PR_SMEM_BYTES;
         cfg.stream = stream;
         cudaLaunchAttribute attr;
         attr.id = cudaLaunchAttributeClusterDimension;
@@ -184,8 +199,9 @@ int launch_tcgen05(bfXcorr p, const void* in, void* out, int accumulate, cudaStr
         attr.val.clusterDim.z = 1;
         cfg.attrs = &attr;
         cfg.numAttrs = 1;
-        e = pair4 ? cudaLaunchKernelEx(&cfg, bfx::xcorr_pair4_kernel, tmap, prm)
-                  : cudaLaunchKernelEx(&cfg, bfx::xcorr_pair_kernel, tmap, prm);
+        e = pair4    ? cudaLaunchKernelEx(&cfg, bfx::xcorr_pair4_kernel, tmap, prm)
+            : stripe ? cudaLaunchKernelEx(&cfg, bfx::xcorr_stripe_kernel, tmap, prm)
+                     : cudaLaunchKernelEx(&cfg, bfx::xcorr_pair_kernel, tmap, prm);
     } else if (few) {
         prm.ntiles = (p->nchan + bfx::FW_NC - 1) / bfx::FW_NC;
         prm.row_in = static_cast<int>(src.row);
@@ -261,6 +277,7 @@ int bfXcorrCreate(bfXcorr* plan, int ninputs, int nchan, int ntime, int dtype)
     const bool pair = ninputs > 64;
     p->pair = pair;
     const int nblk = (ninputs + bfx::PR_BLK - 1) / bfx::PR_BLK;
+    p->stripe = BFX_STRIPE && pair && dtype == BF_XCORR_CI8 && ntime <= bfx::ST_MAXKB * bfx::TC_KT;
     p->tiles_per_chan = pair ? nblk * (nblk + 1) / 2 : 1;
     if (pair && static_cast<unsigned long long>(p->tiles_per_chan) * nchan >= (1ull << 32)) {
         delete p;
@@ -271,13 +288,17 @@ int bfXcorrCreate(bfXcorr* plan, int ninputs, int nchan, int ntime, int dtype)
     if (e == cudaSuccess) e = cudaMemset(p->d_sched, 0, 4 * sizeof(unsigned long long));
     // A channel whose tiles re-read its samples is first rewritten channel-major (S1, tc_relayout_role); with a
     // single tile per channel (ninputs <= 64) every sample is read once anyway and the span is used in place.
-    if (e == cudaSuccess && pair) {
+    // stripes of few row blocks read the span in place (xcorr_stripe.cuh): no ring, no flags
+    const bool direct = p->stripe && nblk <= BFX_DIRECT_MAX_BLK;
+    if (e == cudaSuccess && pair && !direct) {
         // window = channels the grid works on at once (doubled: producers run a tile or two ahead of their loads);
         // on top of that the ring holds ~16 MiB of look-ahead, so a slab is complete long before its first tile is
         // drawn and stays L2-resident until its last tile is done
         const unsigned long long slab = static_cast<unsigned long long>(ntime) * ring_row_bytes(p);
-        const int window = (p->num_sms / 2 + p->tiles_per_chan - 1) / p->tiles_per_chan;
-        long long ahead = static_cast<long long>((16ull << 20) / slab);
+        // (stripe kernel: a pair holds one of the channel's nblk stripes, so more channels are in flight at once)
+        const int per_chan = p->stripe ? nblk : p->tiles_per_chan;
+        const int window = (p->num_sms / 2 + per_chan - 1) / per_chan;
+        long long ahead = static_cast<long long>(((p->stripe ? static_cast<unsigned long long>(BFX_ST_AHEAD_MB) : 16ull) << 20) / slab);
         if (ahead < 2) ahead = 2;
         long long ring = 2 * window + 2 + ahead;
         if (ring > nchan) ring = nchan;
@@ -294,6 +315,8 @@ int bfXcorrCreate(bfXcorr* plan, int ninputs, int nchan, int ntime, int dtype)
         e = cudaFuncSetAttribute(bfx::xcorr_pair4_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bfx::P4_SMEM_BYTES);
     if (e == cudaSuccess)
         e = cudaFuncSetAttribute(bfx::xcorr_pair_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bfx::PR_SMEM_BYTES);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(bfx::xcorr_stripe_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bfx::ST_SMEM_BYTES);
     if (e != cudaSuccess) {
         const int st = cuda_fail(nullptr, e);
         if (p->d_sched) cudaFree(p->d_sched);

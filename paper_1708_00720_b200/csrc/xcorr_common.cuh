@@ -251,6 +251,7 @@ __device__ __forceinline__ void tc_relayout_role(const TcParams& p, uint32_t lan
     const long long src_pitch = static_cast<long long>(p.nchan) * p.row_in;
     const int row_out = p.rl_row_out;  // bytes of one (t, c) row in the ring: 2 N (int8 pairs) or N (packed ci4)
     auto do_unit = [&](int cc, int u) {
+#ifndef BFX_PROBE_RL_ONLY
         if (cc >= p.ring_w) {
             // the slab is still owned by channel cc - ring_w until all of its tiles have loaded their operands
             if (lane == 0) {
@@ -263,6 +264,7 @@ __device__ __forceinline__ void tc_relayout_role(const TcParams& p, uint32_t lan
             }
             __syncwarp();
         }
+#endif
         const int t0 = (u / p.rl_nx) * p.rl_rows;
         const int xb0 = (u % p.rl_nx) * RL_XBYTES;
         const int nt = min(p.rl_rows, p.ntime - t0);
