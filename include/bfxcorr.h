@@ -67,8 +67,8 @@ typedef enum bfXcorrStatus_ {
 
 /* Which kernel bfXcorrExecute launches.  TCGEN05 is the product path and the default: unpack-and-transpose
  * stage, TMA-staged int8 operands, tcgen05.mma kind::i8 with int32 accumulators held in TMEM over the whole span,
- * lower-triangle tile scheduler, span-accumulate epilogue (CTA pairs above 64 inputs, four channels per CTA up to
- * 64 inputs: DESIGN.md section 5).  SIMT is a plain CUDA-core kernel kept as
+ * lower-triangle tile scheduler, span-accumulate epilogue (CTA pairs above 64 inputs -- with a resident A block per
+ * stripe of tiles for ci8 spans of at most 1024 samples --, four channels per CTA up to 64 inputs: DESIGN.md section 5).  SIMT is a plain CUDA-core kernel kept as
  * an on-device cross-check of the tensor path at sizes the CPU oracle cannot reach; it is never
  * selected implicitly. */
 typedef enum bfXcorrAlgo_ {
