@@ -33,6 +33,9 @@ constexpr uint32_t kMagic = 0xBFC0DE01u;
 #ifndef BFX_DIRECT_MAX_BLK
 #define BFX_DIRECT_MAX_BLK 8
 #endif
+#ifndef BFX_DIRECT_STRIDE_KB
+#define BFX_DIRECT_STRIDE_KB 1024
+#endif
 #ifndef BFX_ST_AHEAD_MB
 #define BFX_ST_AHEAD_MB 16
 #endif
@@ -144,7 +147,7 @@ int launch_tcgen05(bfXcorr p, const void* in, void* out, int accumulate, cudaStr
     // operand boxes: 64 inputs x 1 channel x TC_KT samples (128 bytes of int8 pairs); few-input ci4: whole raw rows of
     // FW_NC adjacent channels x FW_KT samples
     const bool pair4 = pair && p->dtype == BF_XCORR_CI4;  // packed ring, unpacked in shared memory
-    const int st = pair4 ? encode_map(p, &tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, src, 1, 64u, CU_TENSOR_MAP_SWIZZLE_NONE, p->ring_w)
+    const int st = pair4 ? encode_map(p, &tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, src, 1, 64u, CU_TENSOR_MAP_SWIZZLE_NONE, fused ? p->ring_w : p->nchan)
                    : few ? encode_map(p, &tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, src, 1, static_cast<unsigned>(src.row),
                                     CU_TENSOR_MAP_SWIZZLE_NONE, p->nchan, bfx::FW_NC, bfx::FW_KT)
                        : encode_map(p, &tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, src, 1, CI4 ? 64u : 128u,
@@ -289,7 +292,11 @@ int bfXcorrCreate(bfXcorr* plan, int ninputs, int nchan, int ntime, int dtype)
     // A channel whose tiles re-read its samples is first rewritten channel-major (S1, tc_relayout_role); with a
     // single tile per channel (ninputs <= 64) every sample is read once anyway and the span is used in place.
     // stripes of few row blocks read the span in place (xcorr_stripe.cuh): no ring, no flags
-    const bool direct = p->stripe && nblk <= BFX_DIRECT_MAX_BLK;
+    // ... and so do ci4 pair spans, and any span whose samples lie close enough together for the TMA's address
+    // translation (BFX_DIRECT_STRIDE_KB between consecutive samples of a channel; cfg2: 128 KiB).  Measured
+    // (profiles/round1.md): with many row blocks AND a stride of 2 MiB or more the S1 ring still wins.
+    const bool near = static_cast<unsigned long long>(nchan) * ninputs * bytes_per_sample(dtype) <= (static_cast<unsigned long long>(BFX_DIRECT_STRIDE_KB) << 10);
+    const bool direct = pair && (p->stripe || dtype == BF_XCORR_CI4) && (nblk <= BFX_DIRECT_MAX_BLK || near);
     if (e == cudaSuccess && pair && !direct) {
         // window = channels the grid works on at once (doubled: producers run a tile or two ahead of their loads);
         // on top of that the ring holds ~16 MiB of look-ahead, so a slab is complete long before its first tile is

@@ -153,7 +153,7 @@ xcorr_pair4_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
             if (w < 0) break;
             const PrWhere tl = pr_decode(w, p.tiles_per_chan);
             const int c = tl.c;
-            if (c != ready_chan) {
+            if (p.z != nullptr && c != ready_chan) {   // (p.z == NULL: the packed span is read in place, no ring)
                 if (lane == 0) {
                     const unsigned long long want = p.epoch * static_cast<unsigned long long>(p.rl_units);
                     uint32_t spins = 0;
@@ -214,7 +214,7 @@ xcorr_pair4_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
                 }
                 if (lane == 0) {
                     ptx::mma_commit_cg2(bar_tfull + 8 * buf, 3);
-                    ptx::red_relaxed_add_u64(p.done + tl.c, 1ull);
+                    if (p.z != nullptr) ptx::red_relaxed_add_u64(p.done + tl.c, 1ull);
                 }
                 __syncwarp();
             }
@@ -322,7 +322,7 @@ xcorr_pair4_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
     } else {
         // ===================== relayout warps (S1): span -> packed ring, a plain copy =====================
         p4_regs_inc<P4_REGS_RELAYOUT>();
-        tc_relayout_role(p, lane);
+        if (p.z != nullptr) tc_relayout_role(p, lane);
     }
 
     ptx::tc_fence_before();
