@@ -28,7 +28,11 @@ constexpr int ST_MAXKB = 8;                          // resident A slots of TC_K
 #define BFX_ST_BSTAGES 4
 #endif
 constexpr int ST_BSTAGES = BFX_ST_BSTAGES;
-constexpr int ST_STG_BYTES = 4 * TC_STG_BUF_BYTES;   // one staging buffer per epilogue warp
+#ifndef BFX_ST_STG_BUFS
+#define BFX_ST_STG_BUFS 1
+#endif
+constexpr int ST_STG_BUFS = BFX_ST_STG_BUFS;          // staging buffers per epilogue warp
+constexpr int ST_STG_BYTES = 4 * ST_STG_BUFS * TC_STG_BUF_BYTES;
 constexpr int ST_SMEM_BYTES = 1024 + (ST_MAXKB + ST_BSTAGES) * TC_BOX_BYTES + ST_STG_BYTES + 512;
 static_assert(ST_SMEM_BYTES <= 232448, "stripe kernel shared memory");
 
@@ -217,7 +221,8 @@ xcorr_stripe_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
     } else if (warp >= 4 && warp < 8) {
         // ===================== epilogue (S4), both CTAs =====================
         const int wq = warp - 4;
-        const uint32_t stg_buf = stg_base + wq * TC_STG_BUF_BYTES;
+        const uint32_t stg_warp = stg_base + wq * ST_STG_BUFS * TC_STG_BUF_BYTES;
+        uint32_t nchunks_done = 0;
         const long long nbl = static_cast<long long>(p.ninputs) * (p.ninputs + 1) / 2;
         uint32_t tcount = 0;
         for (uint32_t it = 0;; ++it) {
@@ -244,9 +249,10 @@ xcorr_stripe_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
                 }
                 ptx::mbar_wait(bar_tfull + 8 * buf, bphase);
                 ptx::tc_fence_after();
-                for (int jc = 0; jc < nchunk; ++jc) {
+                for (int jc = 0; jc < nchunk; ++jc, ++nchunks_done) {
+                    const uint32_t stg_buf = stg_warp + (nchunks_done % ST_STG_BUFS) * TC_STG_BUF_BYTES;
                     const uint32_t tcol = tmem_base + (static_cast<uint32_t>(32 * wq) << 16) + buf * 256 + jc * 128;
-                    tc_epilogue_chunk<false, true, 0>(p, lane, tcol, stg_buf, out_c, i0, j0 + jc * TC_CJ,
+                    tc_epilogue_chunk<false, true, ST_STG_BUFS - 1>(p, lane, tcol, stg_buf, out_c, i0, j0 + jc * TC_CJ,
                                                       jc == nchunk - 1 ? lead_tempty + 8 * buf : 0u);
                 }
             }
