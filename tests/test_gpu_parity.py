@@ -254,3 +254,33 @@ def test_maximum_inputs_32768_sampled():
     last = out[0, (N - 1) * N // 2:(N - 1) * N // 2 + N].cpu().numpy().astype(np.int64)
     jj = np.arange(N)
     np.testing.assert_array_equal(last, oracle.xcorr_entries(x, N, C, T, 8, np.zeros(N, dtype=np.int64), np.full(N, N - 1), jj))
+
+
+@pytest.mark.parametrize("shape", [(512, 300, 1024, 8), (1152, 460, 130, 8), (1152, 920, 130, 4), (512, 256, 300, 4)],
+                         ids=lambda s: "n%dc%dt%dci%d" % s)
+def test_many_launches_on_one_plan_against_the_simt_kernel(shape):
+    """Ten launches on ONE plan, restarting the integration every fourth: the scheduler words, the S1 ring flags and
+    their per-launch epochs are re-used across launches (in-place shapes and shapes that go through the ring).  The
+    reference is the CUDA-core kernel of the same library on the device (itself checked against the oracle above), so
+    shapes far beyond the oracle's reach can be compared in full."""
+    N, C, T, dt = shape
+    dev = torch.device("cuda:0")
+    stream = torch.cuda.current_stream().cuda_stream
+    nb = N * (N + 1) // 2
+    g = torch.Generator(device=dev)
+    g.manual_seed(N + C + T + dt)
+    spans = [torch.randint(0, 256, (T * C * N * (1 if dt == 4 else 2),), dtype=torch.uint8, device=dev, generator=g)
+             for _ in range(3)]
+    outs = []
+    for algo in (bfx.BF_XCORR_ALGO_TCGEN05, bfx.BF_XCORR_ALGO_SIMT):
+        plan = bfx.bfXcorrCreate(N, C, T, dt)
+        try:
+            bfx.bfXcorrSetAlgo(plan, algo)
+            out = torch.full((C, nb, 2), 0x5A5A5A5A, dtype=torch.int32, device=dev)
+            for k in range(10):
+                bfx.bfXcorrExecute(plan, spans[k % 3].data_ptr(), out.data_ptr(), (k % 4) != 0, stream)
+            torch.cuda.synchronize()
+            outs.append(out)
+        finally:
+            bfx.bfXcorrDestroy(plan)
+    assert torch.equal(outs[0], outs[1])
