@@ -48,17 +48,67 @@ def load_peaks():
 
 
 class ClockSampler:
-    """nvidia-smi clocks and throttle reasons sampled DURING the timed region."""
+    """SM clock, power and clock-event (throttle) reasons sampled DURING the timed region.
+
+    NVML is polled in-process every ~2 ms by a thread that is initialised in the constructor, so the first sample
+    falls inside the timed region even when that lasts only tens of milliseconds; `nvidia-smi -lms 50` (which
+    needs ~100 ms to come up) is the fallback when pynvml cannot be used."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
+    NAMES = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
 
     def __init__(self, gpu_index: int):
-        self.rows = []
+        self.rows = []        # nvidia-smi fallback: csv lines
+        self.samples = []     # NVML: (sm_mhz, power_w, reason_mask)
         self.proc = None
         self.gpu = gpu_index
+        self.nvml = None
+        self.handle = None
+        self.sm_max = None
+        self.stop_flag = threading.Event()
+        self.thread = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            try:
+                import torch
+                uuid = str(torch.cuda.get_device_properties(gpu_index).uuid)
+                if not uuid.startswith("GPU-"):
+                    uuid = "GPU-" + uuid
+                self.handle = pynvml.nvmlDeviceGetHandleByUUID(uuid.encode())
+            except Exception:
+                self.handle = pynvml.nvmlDeviceGetHandleByIndex(gpu_index)
+            self.sm_max = float(pynvml.nvmlDeviceGetMaxClockInfo(self.handle, pynvml.NVML_CLOCK_SM))
+            self._poll_once(pynvml)   # fails here, not in the thread, if a query is unsupported
+            self.samples.clear()
+            self.nvml = pynvml
+        except Exception:
+            self.nvml = None
+
+    def _poll_once(self, nv):
+        sm = float(nv.nvmlDeviceGetClockInfo(self.handle, nv.NVML_CLOCK_SM))
+        pw = nv.nvmlDeviceGetPowerUsage(self.handle) / 1000.0
+        try:
+            mask = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.handle))
+        except Exception:
+            mask = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.handle))
+        self.samples.append((sm, pw, mask))
+
+    def _poll(self):
+        nv = self.nvml
+        while not self.stop_flag.is_set():
+            try:
+                self._poll_once(nv)
+            except Exception:
+                break
+            time.sleep(0.002)
 
     def start(self):
+        if self.nvml is not None:
+            self.thread = threading.Thread(target=self._poll, daemon=True)
+            self.thread.start()
+            return
         try:
             self.proc = subprocess.Popen(
                 ["nvidia-smi", "-i", str(self.gpu), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits", "-lms", "50"],
@@ -72,7 +122,25 @@ class ClockSampler:
         for line in self.proc.stdout:
             self.rows.append(line.strip())
 
+    def _stop_nvml(self):
+        self.stop_flag.set()
+        self.thread.join(timeout=2)
+        nv = self.nvml
+        bits = [(nv.nvmlClocksThrottleReasonHwSlowdown, "hw_slowdown"),
+                (nv.nvmlClocksThrottleReasonHwThermalSlowdown, "hw_thermal_slowdown"),
+                (nv.nvmlClocksThrottleReasonSwThermalSlowdown, "sw_thermal_slowdown"),
+                (nv.nvmlClocksThrottleReasonSwPowerCap, "sw_power_cap")]
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.sm_max, "reasons": ["no samples"]}
+        sm_sorted = sorted(s[0] for s in self.samples)
+        reasons = sorted({name for _, _, m in self.samples for bit, name in bits if m & int(bit)})
+        return {"sm_mhz": sm_sorted[len(sm_sorted) // 2], "sm_min_mhz": sm_sorted[0], "sm_max_mhz": self.sm_max,
+                "power_w_max": max(s[1] for s in self.samples), "samples": len(self.samples), "reasons": reasons,
+                "source": "nvml, polled every ~2 ms inside the timed region"}
+
     def stop(self):
+        if self.nvml is not None and self.thread is not None:
+            return self._stop_nvml()
         if not self.proc:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
         time.sleep(0.06)
@@ -82,7 +150,6 @@ class ClockSampler:
         except subprocess.TimeoutExpired:
             self.proc.kill()
         sm, mx, pw, reasons = [], [], [], set()
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         for r in self.rows:
             f = [x.strip() for x in r.split(",")]
             if len(f) < 7:
@@ -91,14 +158,14 @@ class ClockSampler:
                 sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
             except ValueError:
                 continue
-            for n, v in zip(names, f[3:7]):
+            for n, v in zip(self.NAMES, f[3:7]):
                 if v.lower().startswith("active"):
                     reasons.add(n)
         if not sm:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
         sm_sorted = sorted(sm)
         return {"sm_mhz": sm_sorted[len(sm_sorted) // 2], "sm_max_mhz": max(mx), "power_w_max": max(pw),
-                "samples": len(sm), "reasons": sorted(reasons)}
+                "samples": len(sm), "reasons": sorted(reasons), "source": "nvidia-smi -lms 50"}
 
 
 def workload_numbers(cfg):
@@ -221,10 +288,10 @@ def run_beamform(args, cfg):
             if rec is not None:
                 rec.append((e0, e1))
 
+    sampler = ClockSampler(0)
     for _ in range(max(args.warmup, 3)):
         step()
     torch.cuda.synchronize()
-    sampler = ClockSampler(0)
     sampler.start()
     rec = []
     for _ in range(args.steps):
@@ -347,10 +414,10 @@ def main():
             dist.barrier()
             torch.cuda.synchronize()
 
+    sampler = ClockSampler(local_rank) if rank == 0 else None   # NVML comes up here, outside the timed region
     for _ in range(args.warmup):
         step()
     barrier()
-    sampler = ClockSampler(local_rank)
     if rank == 0:
         sampler.start()
     launches = 0
