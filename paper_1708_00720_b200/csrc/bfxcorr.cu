@@ -36,6 +36,14 @@ constexpr uint32_t kMagic = 0xBFC0DE01u;
 #ifndef BFX_DIRECT_STRIDE_KB
 #define BFX_DIRECT_STRIDE_KB 1024
 #endif
+// ci4 pair spans through the S1 ring (0 = always in place).  OFF: with the ring, accumulating launches of
+// xcorr_pair4_kernel lose one epilogue warp's tile now and then (the peer CTA adds it into the tile the pair draws
+// four iterations later; 1152 x 920 x 130 ci4: 25 of 25 runs wrong with accumulate = 1, none with 0, none in place,
+// none with TC_RING 8 or without the epilogue's L2 prefetch: profiles/round1.md).  Not root-caused; until it is, ci4
+// spans are read in place whatever their shape (2048 x 1024 x 1024 ci4: 10.8 ms instead of 8.3).
+#ifndef BFX_P4_RING
+#define BFX_P4_RING 0
+#endif
 #ifndef BFX_ST_AHEAD_MB
 #define BFX_ST_AHEAD_MB 16
 #endif
@@ -296,7 +304,8 @@ int bfXcorrCreate(bfXcorr* plan, int ninputs, int nchan, int ntime, int dtype)
     // translation (BFX_DIRECT_STRIDE_KB between consecutive samples of a channel; cfg2: 128 KiB).  Measured
     // (profiles/round1.md): with many row blocks AND a stride of 2 MiB or more the S1 ring still wins.
     const bool near = static_cast<unsigned long long>(nchan) * ninputs * bytes_per_sample(dtype) <= (static_cast<unsigned long long>(BFX_DIRECT_STRIDE_KB) << 10);
-    const bool direct = pair && (p->stripe || dtype == BF_XCORR_CI4) && (nblk <= BFX_DIRECT_MAX_BLK || near);
+    const bool direct = pair && (p->stripe || dtype == BF_XCORR_CI4) &&
+                        (nblk <= BFX_DIRECT_MAX_BLK || near || (dtype == BF_XCORR_CI4 && !BFX_P4_RING));
     if (e == cudaSuccess && pair && !direct) {
         // window = channels the grid works on at once (doubled: producers run a tile or two ahead of their loads);
         // on top of that the ring holds ~16 MiB of look-ahead, so a slab is complete long before its first tile is

@@ -76,7 +76,10 @@ constexpr int RL_ROWS = BFX_RL_ROWS;      // samples per relayout unit (4 rounds
 constexpr int RL_WARPS = 8;      // relayout warps per CTA
 constexpr int RL_XBYTES = 1024;  // span bytes of one row piece per relayout unit
 
-constexpr int TC_RING = 4;  // depth of the per-CTA ring that passes scheduled tile indices between warp roles
+#ifndef BFX_TC_RING
+#define BFX_TC_RING 4
+#endif
+constexpr int TC_RING = BFX_TC_RING;  // depth of the per-CTA ring that passes scheduled tile indices between warp roles
 
 // UMMA shared-memory descriptor, MN-major, SWIZZLE_128B:
 //   bits [0,14) start >> 4 | [16,30) LBO >> 4 (pitch between 128-byte m-blocks) |

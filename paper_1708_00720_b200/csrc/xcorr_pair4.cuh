@@ -50,12 +50,16 @@ __device__ __forceinline__ void p4_tma_load_hint(uint32_t dst, const CUtensorMap
 template <int N>
 __device__ __forceinline__ void p4_regs_inc()
 {
+#ifndef BFX_P4_NO_SETMAXNREG
     asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N));
+#endif
 }
 template <int N>
 __device__ __forceinline__ void p4_regs_dec()
 {
+#ifndef BFX_P4_NO_SETMAXNREG
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N));
+#endif
 }
 
 __global__ void __launch_bounds__(P4_THREADS, 1)
@@ -251,6 +255,7 @@ xcorr_pair4_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
             int nchunk = (i0 + 15 - j0) / TC_CJ + 1;   // 64-column chunks that reach the diagonal or lie below it
             nchunk = nchunk > 2 ? 2 : nchunk;
             int32_t* const out_c = p.out + 2 * (static_cast<long long>(tl.c) * nbl);
+#ifndef BFX_P4_NO_ACC_PREFETCH
             if (p.accumulate && lane < 16) {
                 // the L2 reduce-adds of this tile will want the old visibilities resident
                 const int i_own = i0 + static_cast<int>(lane);
@@ -262,6 +267,7 @@ xcorr_pair4_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
                     ptx::bulk_prefetch_l2(out_c + 2 * ea, static_cast<uint32_t>(8 * (eb - ea)));
                 }
             }
+#endif
             ptx::mbar_wait(bar_tfull + 8 * buf, bphase);
             ptx::tc_fence_after();
             for (int jc = 0; jc < nchunk; ++jc) {

@@ -32,6 +32,14 @@ constexpr int ST_BSTAGES = BFX_ST_BSTAGES;
 #define BFX_ST_STG_BUFS 1
 #endif
 constexpr int ST_STG_BUFS = BFX_ST_STG_BUFS;          // staging buffers per epilogue warp
+// Tile order inside a stripe.  0: column blocks 0 .. R, the diagonal tile (which loads nothing) last, so a stripe's
+// first tile needs its A and its B boxes at once.  1: the diagonal tile first, so that every tile of a stripe needs
+// exactly one operand block from the L2 (A for the diagonal tile, B for each of the others).
+#ifndef BFX_ST_DIAG_FIRST
+#define BFX_ST_DIAG_FIRST 0
+#endif
+// jj-th tile of a stripe of R + 1 tiles -> column block
+__device__ __forceinline__ int st_col_block(int jj, int R) { return BFX_ST_DIAG_FIRST ? (jj == 0 ? R : jj - 1) : jj; }
 constexpr int ST_STG_BYTES = 4 * ST_STG_BUFS * TC_STG_BUF_BYTES;
 constexpr int ST_SMEM_BYTES = 1024 + (ST_MAXKB + ST_BSTAGES) * TC_BOX_BYTES + ST_STG_BYTES + 512;
 static_assert(ST_SMEM_BYTES <= 232448, "stripe kernel shared memory");
@@ -152,12 +160,13 @@ xcorr_stripe_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
             const int cs = c % p.ring_w;
             const int xa = 256 * R + 128 * static_cast<int>(rank);
             const uint32_t aphase = n & 1;
-            for (int j = 0; j <= R; ++j) {
+            for (int jj = 0; jj <= R; ++jj) {
+                const int j = st_col_block(jj, R);
                 const bool diag = j == R;
                 const int xb = 256 * j + 128 * static_cast<int>(rank);
                 for (int kb = 0; kb < nkb; ++kb) {
                     const int t0 = kb * TC_KT;
-                    if (j == 0) {
+                    if (jj == 0) {
                         ptx::mbar_wait(bar_aempty + 8 * kb, aphase ^ 1);
                         if (lane == 0) {
                             if (leader) ptx::mbar_expect_tx(bar_afull + 8 * kb, 2 * TC_BOX_BYTES);
@@ -187,14 +196,15 @@ xcorr_stripe_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
                 const int c = static_cast<int>(static_cast<uint32_t>(w) / static_cast<uint32_t>(nblk));
                 const int R = nblk - 1 - (static_cast<int>(static_cast<uint32_t>(w)) - c * nblk);
                 const uint32_t aphase = it & 1;
-                for (int j = 0; j <= R; ++j, ++tcount) {
-                    const bool diag = j == R;
+                for (int jj = 0; jj <= R; ++jj, ++tcount) {
+                    const bool diag = st_col_block(jj, R) == R;
+                    const bool last = jj == R;   // the stripe's last tile hands the resident A slots back
                     const uint32_t buf = tcount & 1, bphase = (tcount >> 1) & 1;
                     const uint32_t d_tmem = tmem_base + buf * 256;
                     ptx::mbar_wait(bar_tempty + 8 * buf, bphase ^ 1);
                     ptx::tc_fence_after();
                     for (int kb = 0; kb < nkb; ++kb) {
-                        if (j == 0) ptx::mbar_wait(bar_afull + 8 * kb, aphase);
+                        if (jj == 0) ptx::mbar_wait(bar_afull + 8 * kb, aphase);
                         if (!diag) ptx::mbar_wait(bar_full + 8 * stage, phase);
                         ptx::tc_fence_after();
                         const uint64_t adesc = tc_smem_desc(a_base + kb * TC_BOX_BYTES, TC_BOX_BYTES);
@@ -205,7 +215,7 @@ xcorr_stripe_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
                             for (int k = 0; k < nk; ++k)
                                 ptx::mma_i8<2>(d_tmem, adesc + 256u * k, bdesc + 256u * k, idesc, (kb | k) != 0 ? 1u : 0u);
                             if (!diag) ptx::mma_commit_cg2(bar_empty + 8 * stage, 3);
-                            else ptx::mma_commit_cg2(bar_aempty + 8 * kb, 3);   // the diagonal tile is the stripe's last
+                            if (last) ptx::mma_commit_cg2(bar_aempty + 8 * kb, 3);
                         }
                         __syncwarp();
                         if (!diag && ++stage == S) { stage = 0; phase ^= 1; }
@@ -232,9 +242,9 @@ xcorr_stripe_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
             const int R = nblk - 1 - (static_cast<int>(static_cast<uint32_t>(w)) - c * nblk);
             int32_t* const out_c = p.out + 2 * (static_cast<long long>(c) * nbl);
             const int i0 = PR_BLK * R + 64 * static_cast<int>(rank) + 16 * wq;  // first input row of this warp
-            for (int j = 0; j <= R; ++j, ++tcount) {
+            for (int jj = 0; jj <= R; ++jj, ++tcount) {
                 const uint32_t buf = tcount & 1, bphase = (tcount >> 1) & 1;
-                const int j0 = PR_BLK * j;
+                const int j0 = PR_BLK * st_col_block(jj, R);
                 int nchunk = (i0 + 15 - j0) / TC_CJ + 1;
                 nchunk = nchunk > 2 ? 2 : nchunk;
                 if (p.accumulate && lane < 16) {

@@ -256,13 +256,17 @@ def test_maximum_inputs_32768_sampled():
     np.testing.assert_array_equal(last, oracle.xcorr_entries(x, N, C, T, 8, np.zeros(N, dtype=np.int64), np.full(N, N - 1), jj))
 
 
+@pytest.mark.parametrize("restart", [4, 0], ids=["restart4", "accumulate_always"])
 @pytest.mark.parametrize("shape", [(512, 300, 1024, 8), (1152, 460, 130, 8), (1152, 920, 130, 4), (512, 256, 300, 4)],
                          ids=lambda s: "n%dc%dt%dci%d" % s)
-def test_many_launches_on_one_plan_against_the_simt_kernel(shape):
-    """Ten launches on ONE plan, restarting the integration every fourth: the scheduler words, the S1 ring flags and
-    their per-launch epochs are re-used across launches (in-place shapes and shapes that go through the ring).  The
-    reference is the CUDA-core kernel of the same library on the device (itself checked against the oracle above), so
-    shapes far beyond the oracle's reach can be compared in full."""
+def test_many_launches_on_one_plan_against_the_simt_kernel(shape, restart):
+    """Launches on ONE plan, restarting the integration every fourth or never: the scheduler words, the S1 ring flags
+    and their per-launch epochs are re-used across launches (in-place shapes and shapes that go through the ring).
+    The reference is the CUDA-core kernel of the same library on the device (itself checked against the oracle above),
+    so shapes far beyond the oracle's reach can be compared in full.  The tensor-core side is run three times: the
+    case this test was written after (1152 x 920 x 130 ci4 through the S1 ring, accumulating launches: one epilogue
+    warp's tile lost now and then, profiles/round1.md) was wrong in 40 % of the runs with a restart every fourth
+    launch and in every run without restarts."""
     N, C, T, dt = shape
     dev = torch.device("cuda:0")
     stream = torch.cuda.current_stream().cuda_stream
@@ -271,16 +275,23 @@ def test_many_launches_on_one_plan_against_the_simt_kernel(shape):
     g.manual_seed(N + C + T + dt)
     spans = [torch.randint(0, 256, (T * C * N * (1 if dt == 4 else 2),), dtype=torch.uint8, device=dev, generator=g)
              for _ in range(3)]
-    outs = []
-    for algo in (bfx.BF_XCORR_ALGO_TCGEN05, bfx.BF_XCORR_ALGO_SIMT):
+    nlaunch = 10 if restart else 6
+
+    def run(algo):
         plan = bfx.bfXcorrCreate(N, C, T, dt)
         try:
             bfx.bfXcorrSetAlgo(plan, algo)
             out = torch.full((C, nb, 2), 0x5A5A5A5A, dtype=torch.int32, device=dev)
-            for k in range(10):
-                bfx.bfXcorrExecute(plan, spans[k % 3].data_ptr(), out.data_ptr(), (k % 4) != 0, stream)
+            for k in range(nlaunch):
+                accumulate = (k % restart) != 0 if restart else k > 0
+                bfx.bfXcorrExecute(plan, spans[k % 3].data_ptr(), out.data_ptr(), accumulate, stream)
             torch.cuda.synchronize()
-            outs.append(out)
+            return out
         finally:
             bfx.bfXcorrDestroy(plan)
-    assert torch.equal(outs[0], outs[1])
+
+    ref = run(bfx.BF_XCORR_ALGO_SIMT)
+    for rep in range(3):
+        got = run(bfx.BF_XCORR_ALGO_TCGEN05)
+        assert torch.equal(got, ref), "run %d differs from the CUDA-core kernel" % rep
+        del got
