@@ -36,13 +36,11 @@ constexpr uint32_t kMagic = 0xBFC0DE01u;
 #ifndef BFX_DIRECT_STRIDE_KB
 #define BFX_DIRECT_STRIDE_KB 1024
 #endif
-// ci4 pair spans through the S1 ring (0 = always in place).  OFF: with the ring, accumulating launches of
-// xcorr_pair4_kernel lose one epilogue warp's tile now and then (the peer CTA adds it into the tile the pair draws
-// four iterations later; 1152 x 920 x 130 ci4: 25 of 25 runs wrong with accumulate = 1, none with 0, none in place,
-// none with TC_RING 8 or without the epilogue's L2 prefetch: profiles/round1.md).  Not root-caused; until it is, ci4
-// spans are read in place whatever their shape (2048 x 1024 x 1024 ci4: 10.8 ms instead of 8.3).
+// ci4 pair spans through the S1 ring (0 = always in place; probe knob).  The ring was switched off for a few commits
+// while accumulating launches of xcorr_pair4_kernel lost tiles; the cause was the tile-index ring (PrRing::get in
+// xcorr_pair.cuh: the slot read was not complete before the remote arrival), fixed there: profiles/round1.md.
 #ifndef BFX_P4_RING
-#define BFX_P4_RING 0
+#define BFX_P4_RING 1
 #endif
 #ifndef BFX_ST_AHEAD_MB
 #define BFX_ST_AHEAD_MB 16

@@ -77,6 +77,13 @@ __device__ __forceinline__ void mbar_arrive_cluster_addr(uint32_t cluster_bar)
     asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cluster_bar) : "memory");
 }
 
+// the same with cluster-scope release: this thread's earlier reads and writes are ordered before the arrival for
+// the waiter in the other CTA of the cluster
+__device__ __forceinline__ void mbar_arrive_release_cluster_addr(uint32_t cluster_bar)
+{
+    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_bar) : "memory");
+}
+
 __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity)
 {
     uint32_t ok;

@@ -65,19 +65,53 @@ __device__ __forceinline__ void pr_mbar_wait_cluster(uint32_t bar, uint32_t pari
 
 // The tile ring of a pair: the leader's producer draws an index and writes it into slot n of BOTH CTAs' rings;
 // every consumer role of either CTA reads its local slot and then arrives on the LEADER's "slot free" barrier.
+// Arrival on the leader's sempty after reading a slot.  0 (default): a plain arrival issued AFTER the shuffle that
+// broadcasts the loaded index, i.e. after the load has returned -- a value already in a register cannot be changed by
+// the rewrite that the arrival allows.  2: cluster-scope release from every consumer, 1: from the peer CTA's consumers
+// only -- what the PTX memory model asks for in the letter; measured cost on cfg2 6 - 8 % (2031 / 2070 vs 2204 TOPS),
+// on cfg3 1 - 3 %, with the same 0 wrong runs of 40 as 0 (profiles/round1.md).
+#ifndef BFX_RING_ARRIVE
+#define BFX_RING_ARRIVE 0
+#endif
 struct PrRing {
     uint32_t bar_sfull, ring_base;  // local shared addresses
     uint32_t lead_sempty;           // shared::cluster address of the leader's bar_sempty[0]
 
+    // The slot is rewritten by the leader CTA (a remote store for the peer's copy) as soon as every consumer has
+    // arrived on sempty, so the READ of the slot must be complete before the arrival leaves: lane 0 reads, and the
+    // shuffle that broadcasts the value cannot issue before the load has returned.  (Before: every lane loaded, then
+    // __syncwarp, then lane 0's remote arrival -- which does not wait for the load.  In xcorr_pair4_kernel, whose
+    // unpack warps keep the shared-memory pipe busy, a peer epilogue warp that was the last to arrive now and then
+    // got the index published TC_RING iterations later and added its tile there: profiles/round1.md.)
     template <bool WARP>
     __device__ __forceinline__ long long get(uint32_t n, uint32_t lane) const
     {
         const uint32_t slot = n % TC_RING;
         pr_mbar_wait_cluster(bar_sfull + 8 * slot, (n / TC_RING) & 1);
-        long long w;
-        asm volatile("ld.shared.s64 %0, [%1];" : "=l"(w) : "r"(ring_base + 8 * slot) : "memory");
-        if (WARP) __syncwarp();
-        if (!WARP || lane == 0) ptx::mbar_arrive_cluster_addr(lead_sempty + 8 * slot);
+        long long w = 0;
+        if (!WARP || lane == 0)
+            asm volatile("ld.shared.s64 %0, [%1];" : "=l"(w) : "r"(ring_base + 8 * slot) : "memory");
+#ifdef BFX_RING_DEBUG
+        // probe build: the publisher tags the index with its iteration number (bits 48..62)
+        if ((!WARP || lane == 0) && w >= 0) {
+            const uint32_t tag = static_cast<uint32_t>(w >> 48);
+            if (tag != (n & 0x3FFFu))
+                printf("ring: warp %d rank %u iteration %u read tag %u (w %lld)\n", static_cast<int>(threadIdx.x >> 5),
+                       ptx::cluster_ctarank(), n, tag, w & 0xFFFFFFFFFFFFll);
+            w &= 0xFFFFFFFFFFFFll;
+        }
+#endif
+        if (WARP) w = __shfl_sync(0xffffffffu, w, 0);
+        if (!WARP || lane == 0) {
+#if BFX_RING_ARRIVE == 2
+            ptx::mbar_arrive_release_cluster_addr(lead_sempty + 8 * slot);
+#elif BFX_RING_ARRIVE == 1
+            if (ptx::cluster_ctarank() != 0) ptx::mbar_arrive_release_cluster_addr(lead_sempty + 8 * slot);
+            else ptx::mbar_arrive_cluster_addr(lead_sempty + 8 * slot);   // the leader's own barrier: CTA scope is enough
+#else
+            ptx::mbar_arrive_cluster_addr(lead_sempty + 8 * slot);
+#endif
+        }
         return w;
     }
 };

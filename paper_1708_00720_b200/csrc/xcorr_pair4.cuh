@@ -145,9 +145,14 @@ xcorr_pair4_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
                 if (w >= p.ntiles) w = -1;
                 if (lane == 0) {
                     if (w >= 0) w_next = atomicAdd(p.sched, 1ull);
-                    asm volatile("st.shared.s64 [%0], %1;" ::"r"(ring_base + 8 * slot), "l"(w) : "memory");
+#ifdef BFX_RING_DEBUG
+                    const long long wt = w >= 0 ? (w | (static_cast<long long>(n & 0x3FFFu) << 48)) : w;
+#else
+                    const long long wt = w;
+#endif
+                    asm volatile("st.shared.s64 [%0], %1;" ::"r"(ring_base + 8 * slot), "l"(wt) : "memory");
                     ptx::mbar_arrive(bar_sfull + 8 * slot);
-                    asm volatile("st.shared::cluster.s64 [%0], %1;" ::"r"(ptx::mapa(ring_base + 8 * slot, 1)), "l"(w) : "memory");
+                    asm volatile("st.shared::cluster.s64 [%0], %1;" ::"r"(ptx::mapa(ring_base + 8 * slot, 1)), "l"(wt) : "memory");
                     ptx::mbar_arrive_cluster(bar_sfull + 8 * slot, 1);
                 }
                 w_next = __shfl_sync(0xffffffffu, w_next, 0);
