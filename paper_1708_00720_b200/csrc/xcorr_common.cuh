@@ -125,9 +125,12 @@ struct TcRing {
     {
         const uint32_t slot = n % TC_RING;
         ptx::mbar_wait(bar_sfull + 8 * slot, (n / TC_RING) & 1);
-        long long w;
-        asm volatile("ld.shared.s64 %0, [%1];" : "=l"(w) : "r"(ring_base + 8 * slot) : "memory");
-        if (WARP) __syncwarp();
+        // lane 0 reads; the broadcast cannot issue before the load has returned, so the arrival that lets the
+        // producer rewrite the slot never overtakes the read (see PrRing::get in xcorr_pair.cuh, where it did)
+        long long w = 0;
+        if (!WARP || lane == 0)
+            asm volatile("ld.shared.s64 %0, [%1];" : "=l"(w) : "r"(ring_base + 8 * slot) : "memory");
+        if (WARP) w = __shfl_sync(0xffffffffu, w, 0);
         if (!WARP || lane == 0) ptx::mbar_arrive(bar_sempty + 8 * slot);
         return w;
     }
