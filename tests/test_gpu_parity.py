@@ -257,7 +257,8 @@ def test_maximum_inputs_32768_sampled():
 
 
 @pytest.mark.parametrize("restart", [4, 0], ids=["restart4", "accumulate_always"])
-@pytest.mark.parametrize("shape", [(512, 300, 1024, 8), (1152, 460, 130, 8), (1152, 920, 130, 4), (512, 256, 300, 4)],
+@pytest.mark.parametrize("shape", [(512, 300, 1024, 8), (1152, 460, 130, 8), (1152, 920, 130, 4), (512, 256, 300, 4),
+                                   (1312, 200, 2100, 4), (2048, 64, 700, 4), (1304, 100, 2100, 8), (64, 3000, 1024, 4)],
                          ids=lambda s: "n%dc%dt%dci%d" % s)
 def test_many_launches_on_one_plan_against_the_simt_kernel(shape, restart):
     """Launches on ONE plan, restarting the integration every fourth or never: the scheduler words, the S1 ring flags
