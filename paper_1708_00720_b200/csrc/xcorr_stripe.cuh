@@ -23,7 +23,7 @@
 
 namespace bfx {
 
-constexpr int ST_MAXKB = 8;                          // resident A slots of TC_KT samples: ntime <= 1024
+constexpr int ST_MAXKB = 1024 / TC_KT;               // resident A slots of TC_KT samples: ntime <= 1024 (8 slots of 128)
 #ifndef BFX_ST_BSTAGES
 #define BFX_ST_BSTAGES 4
 #endif
