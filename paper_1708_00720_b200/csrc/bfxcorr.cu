@@ -27,6 +27,9 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
 
 constexpr uint32_t kMagic = 0xBFC0DE01u;
 
+#ifndef BFX_SPAN_PROMO
+#define BFX_SPAN_PROMO CU_TENSOR_MAP_L2_PROMOTION_L2_128B
+#endif
 #ifndef BFX_STRIPE
 #define BFX_STRIPE 1
 #endif
@@ -134,7 +137,7 @@ int encode_map(bfXcorr p, CUtensorMap* m, CUtensorMapDataType type, const Operan
     const cuuint32_t box[3] = {box_elems, box_chan, box_rows};
     const cuuint32_t estr[3] = {1u, 1u, 1u};
     const CUresult r = p->encode(m, type, 3, const_cast<void*>(src.base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                                 swz, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                                 swz, src.base == p->d_z ? CU_TENSOR_MAP_L2_PROMOTION_L2_128B : BFX_SPAN_PROMO, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) {
         p->last_cuda_error = static_cast<int>(cudaErrorInvalidValue);
         return BF_XCORR_DEVICE_ERROR;
@@ -186,7 +189,7 @@ int launch_tcgen05(bfXcorr p, const void* in, void* out, int accumulate, cudaStr
         prm.rl_units = prm.rl_nx * ((p->ntime + rows - 1) / rows);
         prm.ready = p->d_flags;
         prm.done = p->d_flags + p->nchan;
-        prm.epoch = ++p->epoch;
+        prm.epoch = p->epoch + 1;   // committed below, once the launch has been accepted
     }
     cudaError_t e = cudaSuccess;
     if (pair) {
@@ -198,8 +201,16 @@ int launch_tcgen05(bfXcorr p, const void* in, void* out, int accumulate, cudaStr
         cudaLaunchConfig_t cfg;
         std::memset(&cfg, 0, sizeof(cfg));
         cfg.gridDim = dim3(static_cast<unsigned>(2 * pairs));
-        cfg.blockDim = dim3(pair4 ? bfx::P4_THREADS : bfx::PR_THREADS);
-        cfg.dynamicSmemBytes = pair4 ? bfx::P4_SMEM_BYTES : stripe ? bfx::ST_SMEM_BYTES : bfx::PR_SMEM_BYTES;
+        // stripe kernel variants (xcorr_stripe.cuh): through the S1 ring; in place with the register-direct epilogue
+        // (accumulate = 0) or with the staged L2-reduce epilogue (accumulate != 0)
+        using StRing = bfx::StCfg<true, false>;
+        using StDirect = bfx::StCfg<false, true>;
+        using StStaged = bfx::StCfg<false, false>;
+        const int st_variant = !stripe ? -1 : fused ? 0 : accumulate ? 2 : 1;
+        cfg.blockDim = dim3(pair4 ? bfx::P4_THREADS : st_variant == 0 ? StRing::kThreads : st_variant == 1 ? StDirect::kThreads
+                            : st_variant == 2 ? StStaged::kThreads : bfx::PR_THREADS);
+        cfg.dynamicSmemBytes = pair4 ? bfx::P4_SMEM_BYTES : st_variant == 0 ? StRing::kSmemBytes : st_variant == 1 ? StDirect::kSmemBytes
+                               : st_variant == 2 ? StStaged::kSmemBytes : bfx::PR_SMEM_BYTES;
         cfg.stream = stream;
         cudaLaunchAttribute attr;
         attr.id = cudaLaunchAttributeClusterDimension;
@@ -208,9 +219,11 @@ int launch_tcgen05(bfXcorr p, const void* in, void* out, int accumulate, cudaStr
         attr.val.clusterDim.z = 1;
         cfg.attrs = &attr;
         cfg.numAttrs = 1;
-        e = pair4    ? cudaLaunchKernelEx(&cfg, bfx::xcorr_pair4_kernel, tmap, prm)
-            : stripe ? cudaLaunchKernelEx(&cfg, bfx::xcorr_stripe_kernel, tmap, prm)
-                     : cudaLaunchKernelEx(&cfg, bfx::xcorr_pair_kernel, tmap, prm);
+        e = pair4             ? cudaLaunchKernelEx(&cfg, bfx::xcorr_pair4_kernel, tmap, prm)
+            : st_variant == 0 ? cudaLaunchKernelEx(&cfg, bfx::xcorr_stripe_kernel<true, false>, tmap, prm)
+            : st_variant == 1 ? cudaLaunchKernelEx(&cfg, bfx::xcorr_stripe_kernel<false, true>, tmap, prm)
+            : st_variant == 2 ? cudaLaunchKernelEx(&cfg, bfx::xcorr_stripe_kernel<false, false>, tmap, prm)
+                              : cudaLaunchKernelEx(&cfg, bfx::xcorr_pair_kernel, tmap, prm);
     } else if (few) {
         prm.ntiles = (p->nchan + bfx::FW_NC - 1) / bfx::FW_NC;
         prm.row_in = static_cast<int>(src.row);
@@ -219,6 +232,7 @@ int launch_tcgen05(bfXcorr p, const void* in, void* out, int accumulate, cudaStr
     }
     if (e == cudaSuccess) e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(p, e);
+    if (fused) p->epoch += 1;   // the ready[] / done[] counters now run one launch further
     p->last_launch_count += 1;
     return BF_XCORR_OK;
 }
@@ -312,7 +326,7 @@ int bfXcorrCreate(bfXcorr* plan, int ninputs, int nchan, int ntime, int dtype)
         // (stripe kernel: a pair holds one of the channel's nblk stripes, so more channels are in flight at once)
         const int per_chan = p->stripe ? nblk : p->tiles_per_chan;
         const int window = (p->num_sms / 2 + per_chan - 1) / per_chan;
-        long long ahead = static_cast<long long>(((p->stripe ? static_cast<unsigned long long>(BFX_ST_AHEAD_MB) : 16ull) << 20) / slab);
+            long long ahead = static_cast<long long>(((p->stripe ? static_cast<unsigned long long>(BFX_ST_AHEAD_MB) : 16ull) << 20) / slab);
         if (ahead < 2) ahead = 2;
         long long ring = 2 * window + 2 + ahead;
         if (ring > nchan) ring = nchan;
@@ -330,7 +344,11 @@ int bfXcorrCreate(bfXcorr* plan, int ninputs, int nchan, int ntime, int dtype)
     if (e == cudaSuccess)
         e = cudaFuncSetAttribute(bfx::xcorr_pair_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bfx::PR_SMEM_BYTES);
     if (e == cudaSuccess)
-        e = cudaFuncSetAttribute(bfx::xcorr_stripe_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bfx::ST_SMEM_BYTES);
+        e = cudaFuncSetAttribute(bfx::xcorr_stripe_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bfx::StCfg<true, false>::kSmemBytes);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(bfx::xcorr_stripe_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bfx::StCfg<false, true>::kSmemBytes);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(bfx::xcorr_stripe_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bfx::StCfg<false, false>::kSmemBytes);
     if (e != cudaSuccess) {
         const int st = cuda_fail(nullptr, e);
         if (p->d_sched) cudaFree(p->d_sched);

@@ -242,6 +242,103 @@ __device__ __forceinline__ void tc_epilogue_chunk(const TcParams& p, uint32_t la
     }
 }
 
+// ===================== register-direct epilogue (S4): 32 TMEM lanes x 128 columns -> 16 rows x 64 visibilities =====
+// The staged epilogue above hands every row segment to the TMA unit, which it shares with the operand loads: on cfg3
+// its warps spent 47 % of their time in the serialised UBLKCP issue loop (profiles/round2.md).  Here the visibilities go
+// from registers to global memory through the LSU instead, so the TMA unit only loads operands and no staging memory
+// is needed.  tcgen05.ld 16x256b gives thread T (t8 = T / 4, t4 = T % 4) two columns (re_j, im_j) of TMEM lane t8 and of
+// lane t8 + 8; lanes come in (re_i, im_i) pairs, so threads T and T ^ 4 hold the four Gram entries of visibility (i, j)
+// for input row t8 / 2 and for input row t8 / 2 + 4.  One exchange (two shuffles) gives the even-lane thread the
+// complete visibility of the first row and the odd-lane thread that of the second; each stores its 8 bytes, the four
+// threads of a quad covering 32 contiguous bytes of one packed-triangle row.  accumulate != 0: the old values are loaded
+// (8-byte loads issued before the wait for the accumulator, the tile's rows were prefetched into the L2 a tile earlier)
+// and added in registers -- a read-modify-write by the one warp that owns the segment, so no atomics are needed.
+// tcol: TMEM address of (first lane of this warp, first column of the 128-column range).
+__device__ __forceinline__ void tc_release_tmem(uint32_t lane, uint32_t release_bar, bool remote)
+{
+    ptx::tc_fence_before();
+    __syncwarp();
+    if (lane == 0) {
+        if (remote) ptx::mbar_arrive_cluster_addr(release_bar); else ptx::mbar_arrive(release_bar);
+    }
+}
+
+template <bool SHIFT8, bool REMOTE_RELEASE>
+__device__ __forceinline__ void tc_epilogue_direct(const TcParams& p, uint32_t lane, uint32_t tcol, int32_t* out_c, int i0, int jb,
+                                                   uint32_t tfull_bar, uint32_t tfull_phase, uint32_t release_bar)
+{
+    const int t4 = static_cast<int>(lane & 3), t8 = static_cast<int>(lane >> 2);
+    const bool even = (t8 & 1) == 0;
+    const int rowoff = (t8 >> 1) + 4 * (t8 & 1);   // input row of this thread inside an 8-row half
+    int32_t* rowp[2];
+    int rel[2];   // column offset (inside the range, for n = 0) up to which this thread's row has entries: j <= i
+#pragma unroll
+    for (int hh = 0; hh < 2; ++hh) {
+        const int irow = i0 + 8 * hh + rowoff;
+        rowp[hh] = out_c + 2 * (static_cast<long long>(irow) * (irow + 1) / 2 + jb + t4);
+        rel[hh] = irow < p.ninputs ? irow - jb - t4 : -1;
+    }
+    int2 old[2][2][8];
+    if (p.accumulate) {
+#pragma unroll
+        for (int hh = 0; hh < 2; ++hh)
+#pragma unroll
+            for (int cp = 0; cp < 2; ++cp)
+#pragma unroll
+                for (int n = 0; n < 8; ++n) {
+                    const int off = 32 * cp + 4 * n;
+                    old[hh][cp][n] = off <= rel[hh] ? ptx::ld_global_v2(rowp[hh] + 2 * off) : make_int2(0, 0);
+                }
+    }
+    ptx::mbar_wait(tfull_bar, tfull_phase);
+    ptx::tc_fence_after();
+#pragma unroll
+    for (int hh = 0; hh < 2; ++hh) {
+#pragma unroll
+        for (int cp = 0; cp < 2; ++cp) {
+            // warp-uniform: the piece has an entry on or below the diagonal, and its rows exist
+            const bool active = jb + 32 * cp <= i0 + 8 * hh + 7 && i0 + 8 * hh < p.ninputs;
+            uint32_t g[32];
+            if (active) {
+                ptx::tmem_ld_16x256b_x8(tcol + (static_cast<uint32_t>(16 * hh) << 16) + 64 * cp, g);
+                ptx::tmem_ld_wait();
+            }
+            if (hh == 1 && cp == 1 && release_bar) tc_release_tmem(lane, release_bar, REMOTE_RELEASE);   // this warp's TMEM reads are done
+            if (active) {
+#pragma unroll
+                for (int n = 0; n < 8; ++n) {
+                    const int a0 = static_cast<int>(g[4 * n]), a1 = static_cast<int>(g[4 * n + 1]);
+                    const int b0 = static_cast<int>(g[4 * n + 2]), b1 = static_cast<int>(g[4 * n + 3]);
+                    // even lanes (re rows) keep lane t8's pair and send lane t8 + 8's; odd lanes (im rows) the reverse
+                    const int x0 = __shfl_xor_sync(0xffffffffu, even ? b0 : a0, 4);
+                    const int x1 = __shfl_xor_sync(0xffffffffu, even ? b1 : a1, 4);
+                    // Re V = G[re_i][re_j] + G[im_i][im_j],  Im V = G[im_i][re_j] - G[re_i][im_j]
+                    int re = (even ? a0 : b1) + (even ? x1 : x0);
+                    int im = (even ? x0 : b0) - (even ? a1 : x1);
+                    if (SHIFT8) { re >>= 8; im >>= 8; }   // G came out scaled by 16 * 16, exactly
+                    const int off = 32 * cp + 4 * n;
+                    if (p.accumulate) { re += old[hh][cp][n].x; im += old[hh][cp][n].y; }
+                    if (off <= rel[hh]) ptx::st_global_v2(rowp[hh] + 2 * off, make_int2(re, im));
+                }
+            }
+        }
+    }
+}
+
+// accumulate != 0: pull the old visibilities of (16 rows from i0) x (columns j0 .. j0 + ncol) into the L2 ahead of
+// the loads of tc_epilogue_direct.  Lane l covers half of row i0 + l / 2.
+__device__ __forceinline__ void tc_prefetch_old(const TcParams& p, uint32_t lane, const int32_t* out_c, int i0, int j0, int ncol)
+{
+    const int irow = i0 + static_cast<int>(lane >> 1);
+    int n = irow + 1 - j0;
+    n = n > ncol ? ncol : n;
+    if (irow >= p.ninputs || n <= 0) return;
+    const char* const beg = reinterpret_cast<const char*>(out_c + 2 * (static_cast<long long>(irow) * (irow + 1) / 2 + j0));
+    const char* const end = beg + 8 * n;
+    const char* q = reinterpret_cast<const char*>(reinterpret_cast<uintptr_t>(beg) & ~static_cast<uintptr_t>(127)) + 128 * (lane & 1);
+    for (; q < end; q += 256) ptx::prefetch_l2_line(q);
+}
+
 // ===================== relayout warps (S1: unpack-and-transpose, span -> ring z) =====================
 // Shared by the 1-CTA and the CTA-pair kernels; run by whole warps.
 __device__ __forceinline__ void tc_relayout_role(const TcParams& p, uint32_t lane)

@@ -18,42 +18,50 @@
 // Barriers per CTA: a_full[kb] / a_empty[kb] per resident slot (phase = stripe parity), b_full / b_empty per ring
 // stage, tfull / tempty per accumulator, the stripe-index ring.  A slot kb is released by a commit after the LAST
 // tile's MMAs on it, so the next stripe's A loads trail the current stripe's last tile by one slot.
+//
+// Epilogue (S4), chosen per launch (profiles/round2.md):
+//   accumulate = 0, span in place: tc_epilogue_direct by EIGHT warps (warp 4 + 4 h + q drains TMEM lane quarter q,
+//     column half h) -- registers -> 8-byte global stores through the LSU.  The staged epilogue's warps spent 47 % of
+//     their time in the serialised bulk-copy issue loop, competing with the operand loads for the TMA unit; without
+//     staging memory there is room for six B stages.
+//   accumulate != 0, or operands through the S1 ring: tc_epilogue_chunk by four warps -- staged rows, added at the L2 by
+//     cp.reduce.async.bulk (a read-modify-write through the SM was measured slower: 3.3 against 2.15 ms on cfg3).
 #pragma once
 #include "xcorr_pair.cuh"
 
 namespace bfx {
 
 constexpr int ST_MAXKB = 1024 / TC_KT;               // resident A slots of TC_KT samples: ntime <= 1024 (8 slots of 128)
-#ifndef BFX_ST_BSTAGES
-#define BFX_ST_BSTAGES 4
-#endif
-constexpr int ST_BSTAGES = BFX_ST_BSTAGES;
-#ifndef BFX_ST_STG_BUFS
-#define BFX_ST_STG_BUFS 1
-#endif
-constexpr int ST_STG_BUFS = BFX_ST_STG_BUFS;          // staging buffers per epilogue warp
-// Tile order inside a stripe.  0: column blocks 0 .. R, the diagonal tile (which loads nothing) last, so a stripe's
-// first tile needs its A and its B boxes at once.  1: the diagonal tile first, so that every tile of a stripe needs
-// exactly one operand block from the L2 (A for the diagonal tile, B for each of the others).
-#ifndef BFX_ST_DIAG_FIRST
-#define BFX_ST_DIAG_FIRST 0
-#endif
-// jj-th tile of a stripe of R + 1 tiles -> column block
-__device__ __forceinline__ int st_col_block(int jj, int R) { return BFX_ST_DIAG_FIRST ? (jj == 0 ? R : jj - 1) : jj; }
-constexpr int ST_STG_BYTES = 4 * ST_STG_BUFS * TC_STG_BUF_BYTES;
-constexpr int ST_SMEM_BYTES = 1024 + (ST_MAXKB + ST_BSTAGES) * TC_BOX_BYTES + ST_STG_BYTES + 512;
-static_assert(ST_SMEM_BYTES <= 232448, "stripe kernel shared memory");
 
-__global__ void __launch_bounds__(PR_THREADS, 1)
+// RING: operands through the S1 ring (8 relayout warps); DIRECT_EPI: the register-direct epilogue (in place, accumulate = 0)
+template <bool RING, bool DIRECT_EPI>
+struct StCfg {
+    static_assert(!(RING && DIRECT_EPI), "the register-direct epilogue is built for the in-place kernel only");
+    static constexpr int kBStages = DIRECT_EPI ? 6 : 4;
+    static constexpr int kEpiWarps = DIRECT_EPI ? 8 : 4;
+    static constexpr int kThreads = DIRECT_EPI ? 32 * (4 + kEpiWarps) : 512;   // staged variants: warps 8..15 relayout (RING) or idle
+    static constexpr int kStgBytes = DIRECT_EPI ? 0 : 4 * TC_STG_BUF_BYTES;   // one staging buffer per epilogue warp
+    static constexpr int kSmemBytes = 1024 + (ST_MAXKB + kBStages) * TC_BOX_BYTES + kStgBytes + 512;
+    static_assert(kSmemBytes <= 232448, "stripe kernel shared memory");
+};
+
+// jj-th tile of a stripe of R + 1 tiles -> column block: 0 .. R, the diagonal tile (which loads nothing) last.  (The
+// diagonal tile first, so that every tile needs exactly one operand block, changed nothing: profiles/round1.md.)
+__device__ __forceinline__ int st_col_block(int jj, int /*R*/) { return jj; }
+
+template <bool RING, bool DIRECT_EPI>
+__global__ void __launch_bounds__(StCfg<RING, DIRECT_EPI>::kThreads, 1)
 xcorr_stripe_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
 {
-    constexpr int S = ST_BSTAGES;
+    using Cfg = StCfg<RING, DIRECT_EPI>;
+    constexpr int S = Cfg::kBStages;
+    constexpr int EPI_WARPS = Cfg::kEpiWarps;
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
     const uint32_t a_base = smem_base;                               // ST_MAXKB resident A-half boxes
     const uint32_t b_base = a_base + ST_MAXKB * TC_BOX_BYTES;        // S streaming B-half boxes
     const uint32_t stg_base = b_base + S * TC_BOX_BYTES;             // epilogue staging
-    const uint32_t bar_base = stg_base + ST_STG_BYTES;
+    const uint32_t bar_base = stg_base + Cfg::kStgBytes;
     const uint32_t bar_afull = bar_base;                     // [ST_MAXKB] leader: both CTAs' A boxes have landed
     const uint32_t bar_aempty = bar_afull + 8 * ST_MAXKB;    // [ST_MAXKB] both: the stripe's last MMAs on the slot are done
     const uint32_t bar_full = bar_aempty + 8 * ST_MAXKB;     // [S] leader: both CTAs' B boxes have landed
@@ -82,11 +90,11 @@ xcorr_stripe_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
         }
         for (int b = 0; b < 2; ++b) {
             ptx::mbar_init(bar_tfull + 8 * b, 1);
-            ptx::mbar_init(bar_tempty + 8 * b, 8);
+            ptx::mbar_init(bar_tempty + 8 * b, 2 * EPI_WARPS);   // drained by the epilogue warps of the pair
         }
         for (int s = 0; s < TC_RING; ++s) {
             ptx::mbar_init(bar_sfull + 8 * s, 1);
-            ptx::mbar_init(bar_sempty + 8 * s, 10);
+            ptx::mbar_init(bar_sempty + 8 * s, 2 + 2 * EPI_WARPS);   // leader: MMA issuer + epilogue; peer: producer + epilogue
         }
         ptx::fence_barrier_init();
     }
@@ -103,7 +111,7 @@ xcorr_stripe_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
 
     const int nkb = (p.ntime + TC_KT - 1) / TC_KT;
     const int nblk = (p.ninputs + PR_BLK - 1) / PR_BLK;
-    const bool direct = p.z == nullptr;   // operands straight from the span: no ring, no relayout (see the header)
+    constexpr bool direct = !RING;        // operands straight from the span: no ring, no relayout (see the header)
     const PrRing ring{bar_sfull, ring_base, ptx::mapa(bar_sempty, 0)};
     const uint32_t lead_full = ptx::mapa(bar_full, 0);
     const uint32_t lead_afull = ptx::mapa(bar_afull, 0);
@@ -127,9 +135,6 @@ xcorr_stripe_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
                 ptx::mbar_wait(bar_sempty + 8 * slot, ((n / TC_RING) & 1) ^ 1);
                 w = static_cast<long long>(w_next);
                 if (w >= p.ntiles) w = -1;
-#ifdef BFX_PROBE_RL_ONLY
-                w = -1;
-#endif
                 if (lane == 0) {
                     if (w >= 0) w_next = atomicAdd(p.sched, 1ull);
                     asm volatile("st.shared.s64 [%0], %1;" ::"r"(ring_base + 8 * slot), "l"(w) : "memory");
@@ -139,19 +144,17 @@ xcorr_stripe_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
                 }
                 w_next = __shfl_sync(0xffffffffu, w_next, 0);
             } else {
-                w = __shfl_sync(0xffffffffu, ring.get<true>(n, lane), 0);
+                w = __shfl_sync(0xffffffffu, ring.template get<true>(n, lane), 0);
             }
             if (w < 0) break;
             const int c = static_cast<int>(static_cast<uint32_t>(w) / static_cast<uint32_t>(nblk));
             const int R = nblk - 1 - (static_cast<int>(static_cast<uint32_t>(w)) - c * nblk);
             if (!direct && c != ready_chan) {
                 if (lane == 0) {
-#ifndef BFX_PROBE_NO_RL
                     const unsigned long long want = p.epoch * static_cast<unsigned long long>(p.rl_units);
                     uint32_t spins = 0;
                     while (ptx::ld_acquire_u64(p.ready + c) < want)
                         if (++spins > (1u << 26)) __trap();
-#endif
                     ptx::fence_proxy_async_global();
                 }
                 __syncwarp();
@@ -191,7 +194,7 @@ xcorr_stripe_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
             uint32_t stage = 0, phase = 0, tcount = 0;
             const uint32_t idesc = tc_instr_desc(256, 256);
             for (uint32_t it = 0;; ++it) {
-                const long long w = __shfl_sync(0xffffffffu, ring.get<true>(it, lane), 0);
+                const long long w = __shfl_sync(0xffffffffu, ring.template get<true>(it, lane), 0);
                 if (w < 0) break;
                 const int c = static_cast<int>(static_cast<uint32_t>(w) / static_cast<uint32_t>(nblk));
                 const int R = nblk - 1 - (static_cast<int>(static_cast<uint32_t>(w)) - c * nblk);
@@ -228,15 +231,14 @@ xcorr_stripe_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
                 }
             }
         }
-    } else if (warp >= 4 && warp < 8) {
+    } else if (warp >= 4 && warp < 4 + EPI_WARPS) {
         // ===================== epilogue (S4), both CTAs =====================
-        const int wq = warp - 4;
-        const uint32_t stg_warp = stg_base + wq * ST_STG_BUFS * TC_STG_BUF_BYTES;
-        uint32_t nchunks_done = 0;
+        const int wq = warp & 3;                       // TMEM lane quarter of this warp
         const long long nbl = static_cast<long long>(p.ninputs) * (p.ninputs + 1) / 2;
         uint32_t tcount = 0;
+        [[maybe_unused]] uint32_t nchunks_done = 0;
         for (uint32_t it = 0;; ++it) {
-            const long long w = ring.get<true>(it, lane);
+            const long long w = ring.template get<true>(it, lane);
             if (w < 0) break;
             const int c = static_cast<int>(static_cast<uint32_t>(w) / static_cast<uint32_t>(nblk));
             const int R = nblk - 1 - (static_cast<int>(static_cast<uint32_t>(w)) - c * nblk);
@@ -245,31 +247,48 @@ xcorr_stripe_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
             for (int jj = 0; jj <= R; ++jj, ++tcount) {
                 const uint32_t buf = tcount & 1, bphase = (tcount >> 1) & 1;
                 const int j0 = PR_BLK * st_col_block(jj, R);
-                int nchunk = (i0 + 15 - j0) / TC_CJ + 1;
-                nchunk = nchunk > 2 ? 2 : nchunk;
-                if (p.accumulate && lane < 16) {
-                    const int i_own = i0 + static_cast<int>(lane);
-                    int n = i_own + 1 - j0;
-                    n = n > PR_BLK ? PR_BLK : n;
-                    if (i_own < p.ninputs && n > 0) {
-                        const long long e0 = static_cast<long long>(i_own) * (i_own + 1) / 2 + j0;
-                        const long long ea = e0 & ~1ll, eb = (e0 + n + 1) & ~1ll;
-                        ptx::bulk_prefetch_l2(out_c + 2 * ea, static_cast<uint32_t>(8 * (eb - ea)));
+                if constexpr (DIRECT_EPI) {
+                    const int h = (warp - 4) >> 2;         // the 128-column half this warp drains
+                    const int jb = j0 + 64 * h;
+                    if (jb <= i0 + 15) {   // its 16 rows x 64 columns reach the diagonal or lie below it (warp-uniform)
+                        const uint32_t tcol = tmem_base + (static_cast<uint32_t>(32 * wq) << 16) + buf * 256 + h * 128;
+                        tc_epilogue_direct<false, true>(p, lane, tcol, out_c, i0, jb, bar_tfull + 8 * buf, bphase, lead_tempty + 8 * buf);
+                    } else {
+                        // nothing to store, but the accumulator may only be handed back once it is complete (the MMA
+                        // issuer counts one arrival per warp and tile)
+                        ptx::mbar_wait(bar_tfull + 8 * buf, bphase);
+                        tc_release_tmem(lane, lead_tempty + 8 * buf, true);
                     }
-                }
-                ptx::mbar_wait(bar_tfull + 8 * buf, bphase);
-                ptx::tc_fence_after();
-                for (int jc = 0; jc < nchunk; ++jc, ++nchunks_done) {
-                    const uint32_t stg_buf = stg_warp + (nchunks_done % ST_STG_BUFS) * TC_STG_BUF_BYTES;
-                    const uint32_t tcol = tmem_base + (static_cast<uint32_t>(32 * wq) << 16) + buf * 256 + jc * 128;
-                    tc_epilogue_chunk<false, true, ST_STG_BUFS - 1>(p, lane, tcol, stg_buf, out_c, i0, j0 + jc * TC_CJ,
-                                                      jc == nchunk - 1 ? lead_tempty + 8 * buf : 0u);
+                } else {
+                    const uint32_t stg_warp = stg_base + wq * TC_STG_BUF_BYTES;
+                    int nchunk = (i0 + 15 - j0) / TC_CJ + 1;
+                    nchunk = nchunk > 2 ? 2 : nchunk;
+                    if (p.accumulate && lane < 16) {
+                        // the L2 reduce-adds of this tile will want the old visibilities resident
+                        const int i_own = i0 + static_cast<int>(lane);
+                        int n = i_own + 1 - j0;
+                        n = n > PR_BLK ? PR_BLK : n;
+                        if (i_own < p.ninputs && n > 0) {
+                            const long long e0 = static_cast<long long>(i_own) * (i_own + 1) / 2 + j0;
+                            const long long ea = e0 & ~1ll, eb = (e0 + n + 1) & ~1ll;
+                            ptx::bulk_prefetch_l2(out_c + 2 * ea, static_cast<uint32_t>(8 * (eb - ea)));
+                        }
+                    }
+                    ptx::mbar_wait(bar_tfull + 8 * buf, bphase);
+                    ptx::tc_fence_after();
+                    for (int jc = 0; jc < nchunk; ++jc, ++nchunks_done) {
+                        const uint32_t tcol = tmem_base + (static_cast<uint32_t>(32 * wq) << 16) + buf * 256 + jc * 128;
+                        tc_epilogue_chunk<false, true, 0>(p, lane, tcol, stg_warp, out_c, i0, j0 + jc * TC_CJ,
+                                                          jc == nchunk - 1 ? lead_tempty + 8 * buf : 0u);
+                    }
                 }
             }
         }
-        if (lane < 16) ptx::bulk_wait_read<0>();
-    } else if (warp >= 8) {
-        if (!direct) tc_relayout_role(p, lane);
+        if constexpr (!DIRECT_EPI) {
+            if (lane < 16) ptx::bulk_wait_read<0>();   // shared memory must outlive the bulk reads
+        }
+    } else if (RING && warp >= 8) {
+        tc_relayout_role(p, lane);
     }
 
     ptx::tc_fence_before();
