@@ -14,8 +14,15 @@ e2e         same metric through bfXcorrExecuteHost: pinned HOST spans copied in 
             buffer copied back inside the timed region
 roofline    dominant kernel (the only kernel): algorithmic ops (and bytes) per launch / mean launch
             duration from CUDA events on the launching stream, against MEASURED_PEAKS.json
+            roofline.same_mix_peak: what a no-math streaming kernel with the step's read : write mix
+            (bfXcorrMemoryProbe) reaches in the same run -- the HBM ceiling of this access mix on this box
 cpu_baseline the CPU oracle (oracle/, as it stands) timed on this box's host cores on a bounded
-            sample of the same workload -- a baseline, not the target
+            sample of the same workload -- a baseline, not the target; one_thread: its per-core rate
+parity      the buffer the TIMED launches left behind, compared bit for bit with the oracle on the
+            channels the cpu_baseline leg computed
+ms_per_step mean over the timed region; ms_per_step_median / _min: per-step sums of the launch durations
+sustained   the same step back to back for >= 1 s with its own clock record (the default timed region
+            ends before the board reaches its power cap)
 N > 1       channels are independent: every rank runs the same per-GPU workload on
             its own GPU with no collective on the data path ("weak" scaling); time = max over ranks.
 """
@@ -190,31 +197,44 @@ def config_dict(cfg, extra=None):
     return d
 
 
+def spaced_channels(nchan: int, n: int):
+    return sorted(set(int(round(k * (nchan - 1) / max(1, n - 1))) for k in range(n))) if n > 1 else [0]
+
+
 def oracle_sample(cfg, target_s: float):
-    """Time the oracle (as it stands) on a bounded channel subset of the workload.
-    Returns (seconds, nchannels_used, threads)."""
-    import numpy as np
+    """Time the oracle (as it stands) on a bounded channel subset of the workload, all spans accumulated.
+    Returns (seconds, channels, threads, oracle result [len(channels)][B][2], one-thread info)."""
     import oracle
     from xcorr_inputs import generate_channel_slab
     nthreads = oracle.threads()
     # calibration: one channel per thread, one span
-    ncal = min(cfg.nchan, nthreads)
-    chans = [int(round(k * (cfg.nchan - 1) / max(1, ncal - 1))) for k in range(ncal)] if ncal > 1 else [0]
+    chans = spaced_channels(cfg.nchan, min(cfg.nchan, nthreads))
     x = generate_channel_slab(cfg, 0, chans).numpy()
     t0 = time.perf_counter()
     oracle.xcorr(x, cfg.ninputs, len(chans), cfg.ntime, cfg.dtype)
     tcal = time.perf_counter() - t0
-    per_chan_span = tcal / len(chans) * min(len(chans), nthreads)  # seconds of one "wave" of nthreads channels
-    waves = max(1, int(target_s / max(per_chan_span * cfg.nspans, 1e-9)))
-    nch = min(cfg.nchan, waves * nthreads)
-    chans = sorted(set(int(round(k * (cfg.nchan - 1) / max(1, nch - 1))) for k in range(nch))) if nch > 1 else [0]
+    per_wave = tcal / len(chans) * min(len(chans), nthreads)  # seconds of one "wave" of nthreads channels, one span
+    waves = max(1, int(target_s / max(per_wave * cfg.nspans, 1e-9)))
+    chans = spaced_channels(cfg.nchan, min(cfg.nchan, waves * nthreads))
     slabs = [generate_channel_slab(cfg, s, chans).numpy() for s in range(cfg.nspans)]
     t0 = time.perf_counter()
     out = oracle.xcorr(slabs[0], cfg.ninputs, len(chans), cfg.ntime, cfg.dtype)
     for s in range(1, cfg.nspans):
         oracle.xcorr(slabs[s], cfg.ninputs, len(chans), cfg.ntime, cfg.dtype, out=out, accumulate=True)
     dt = time.perf_counter() - t0
-    return dt, len(chans), nthreads
+    # per-core rate (BASELINE.md section 4): the same oracle on one thread, one channel, one span
+    one = None
+    try:
+        oracle.set_threads(1)
+        x1 = slabs[0][:, :1].copy()
+        t0 = time.perf_counter()
+        oracle.xcorr(x1, cfg.ninputs, 1, cfg.ntime, cfg.dtype)
+        d1 = time.perf_counter() - t0
+        one = {"value": 8.0 * cfg.ntime * cfg.nbaselines / d1 / 1e12, "unit": "TOPS", "cores": 1,
+               "sample": "1 channel, 1 span; %.3f s" % d1}
+    finally:
+        oracle.set_threads(nthreads)
+    return dt, chans, nthreads, out, one
 
 
 def run_reference(args, cfg):
@@ -351,7 +371,9 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
-    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--e2e-steps", type=int, default=8, help="steps of the end-to-end leg (enough that pipeline fill and drain do not dominate)")
+    ap.add_argument("--sustain-seconds", type=float, default=1.0, help="length of the sustained run reported as `sustained` (0 = skip)")
+    ap.add_argument("--no-probe", action="store_true", help="skip the same-mix memory probe")
     ap.add_argument("--op", default="xcorr", choices=["xcorr", "beamform"],
                     help="xcorr: the hot path (the driver's line); beamform: the second workload on the same spans "
                          "(SURVEY.md 8f N1), 1 GPU, its own JSON line")
@@ -368,6 +390,17 @@ def main():
         run_reference(args, cfg)
         return
 
+    # --gpus N without a launcher: start the N ranks here (one process per GPU, torch.distributed.run does the
+    # rendezvous on 127.0.0.1); under torchrun the environment already carries RANK / WORLD_SIZE
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        import socket
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        raise SystemExit(subprocess.call(cmd))
+
     import torch
     import paper_1708_00720_b200 as bfx
 
@@ -376,6 +409,10 @@ def main():
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the X-engine has no CPU fallback")
+    if world != args.gpus:
+        raise SystemExit("bench.py --gpus %d was started with WORLD_SIZE=%d" % (args.gpus, world))
+    if local_rank >= torch.cuda.device_count():
+        raise SystemExit("bench.py: rank %d has no GPU (%d visible)" % (local_rank, torch.cuda.device_count()))
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
     dist = None
@@ -414,6 +451,13 @@ def main():
             dist.barrier()
             torch.cuda.synchronize()
 
+    def max_over_ranks(v):
+        if dist is None:
+            return v
+        t = torch.tensor([v], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
     sampler = ClockSampler(local_rank) if rank == 0 else None   # NVML comes up here, outside the timed region
     for _ in range(args.warmup):
         step()
@@ -429,18 +473,70 @@ def main():
     t_end.record(stream)
     barrier()
     clocks = sampler.stop() if rank == 0 else None
-    total_ms = t_begin.elapsed_time(t_end)
-    if dist is not None:
-        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks(t_begin.elapsed_time(t_end))
     ms_per_step = total_ms / args.steps
     per_span_ms = {}
     for s, e0, e1 in rec:
         per_span_ms.setdefault(s, []).append(e0.elapsed_time(e1))
     launch_ms = [sum(v) / len(v) for _, v in sorted(per_span_ms.items())]
     mean_launch_ms = sum(sum(v) for v in per_span_ms.values()) / max(1, sum(len(v) for v in per_span_ms.values()))
+    # per-step kernel time (sum over the step's launches), for the median / min (>= 20 repetitions)
+    step_ms = sorted(sum(per_span_ms[s][k] for s in per_span_ms) for k in range(args.steps))
     timed_launches = launches
+    kernel_names = sorted({bfx.bfXcorrGetKernelName(plan, s > 0) for s in range(cfg.nspans)})
+
+    # ---- parity on the TIMED kernel's output: `out` now holds the last timed step (all spans accumulated)
+    parity, cpu = None, None
+    if rank == 0 and not args.no_cpu_baseline:
+        dt, chans, nthreads, exp, one = oracle_sample(cfg, args.cpu_seconds)
+        frac = len(chans) / cfg.nchan
+        got = out[torch.tensor(chans, device=dev)].cpu()
+        equal = bool(torch.equal(got, torch.from_numpy(exp)))
+        parity = {"channels": len(chans), "of": cfg.nchan, "equal": equal,
+                  "what": "every visibility of the sampled channels after the last timed step, bit for bit against the oracle"}
+        cpu = {"value": wl["ops_step"] * frac / dt / 1e12, "unit": "TOPS", "cores": nthreads, "kind": "oracle",
+               "sample": "%d of %d channels (evenly spaced), all %d span(s), full ntime and ninputs; %.1f s" % (
+                   len(chans), cfg.nchan, cfg.nspans, dt),
+               "samples_per_s": wl["samples_step"] * frac / dt, "one_thread": one}
+        del got, exp
+
+    # ---- sustained: the same step back to back for >= sustain seconds, with its own clock record
+    sustained = None
+    if args.sustain_seconds > 0:
+        n_sus = max(args.steps, int(args.sustain_seconds * 1e3 / ms_per_step) + 1)
+        s_sampler = ClockSampler(local_rank) if rank == 0 else None
+        barrier()
+        if rank == 0:
+            s_sampler.start()
+        a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        for _ in range(n_sus):
+            step()
+        b.record(stream)
+        barrier()
+        s_clocks = s_sampler.stop() if rank == 0 else None
+        s_ms = max_over_ranks(a.elapsed_time(b)) / n_sus
+        sustained = {"value": wl["ops_step"] * world / (s_ms * 1e-3) / 1e12, "unit": "TOPS", "ms_per_step": s_ms,
+                     "steps": n_sus, "clocks": s_clocks}
+
+    # ---- the same-mix HBM ceiling: a no-math streaming kernel moving the step's algorithmic bytes
+    same_mix = None
+    if rank == 0 and not args.no_probe:
+        probe_ms = []
+        for s in range(cfg.nspans):
+            ts = []
+            for k in range(5):
+                e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+                bfx.bfXcorrMemoryProbe(plan, spans[s].data_ptr(), out.data_ptr(), s > 0, sptr)
+                e1.record(stream)
+                torch.cuda.synchronize()
+                if k >= 2:
+                    ts.append(e0.elapsed_time(e1))
+            probe_ms.append(sum(ts) / len(ts))
+        same_mix = {"gbs": wl["bytes_step"] / (sum(probe_ms) * 1e-3) / 1e9, "launch_ms": probe_ms,
+                    "kernel": "mem_probe_kernel (reads the span, writes / read-modify-writes the visibilities, no math)"}
+    barrier()
 
     # ---- end to end through the host-buffer entry point
     e2e = None
@@ -466,12 +562,7 @@ def main():
                 e2e_step()
             b.record(stream)
             barrier()
-            e_ms = a.elapsed_time(b)
-            if dist is not None:
-                t = torch.tensor([e_ms], dtype=torch.float64, device=dev)
-                dist.all_reduce(t, op=dist.ReduceOp.MAX)
-                e_ms = float(t.item())
-            e_ms /= args.e2e_steps
+            e_ms = max_over_ranks(a.elapsed_time(b)) / args.e2e_steps
             e2e = {"value": wl["ops_step"] * world / (e_ms * 1e-3) / 1e12, "unit": "TOPS",
                    "h2d_bytes_per_step": int(cfg.span_bytes * cfg.nspans), "d2h_bytes_per_step": int(cfg.out_bytes),
                    "ms_per_step": e_ms, "steps": args.e2e_steps,
@@ -515,10 +606,7 @@ def main():
     roofline["peak_source"] = "%s (%s; int8 = 2 x bf16 %s)" % (
         peaks["source"], "MEASURED_PEAKS.json" if peaks["source"] == "measured" else "B200_PROFILING.md fallback",
         "sustained" if long_region else "burst")
-    roofline["kernel"] = ("xcorr_simt_kernel" if args.algo != "tcgen05" else
-                          ("xcorr_pair4_kernel" if cfg.dtype == 4 else
-                           "xcorr_stripe_kernel" if cfg.ntime <= 1024 else "xcorr_pair_kernel") if cfg.ninputs > 64
-                          else "xcorr_few_kernel")
+    roofline["kernel"] = "; ".join(kernel_names)   # bfXcorrGetKernelName: the dispatch rule lives in the library
     # context: tcgen05.mma kind::i8 issue-rate probe on this pool (profiles/round1.md): 8192 MAC/clk/SM -> 4.6 POPS at 1.9 GHz
     roofline["int8_mma_probe_peak_tops"] = 4610.0
     roofline["launch_ms"] = launch_ms
@@ -526,15 +614,11 @@ def main():
     roofline["algorithmic_bytes_per_launch"] = bytes_launch
     roofline["other_bound"] = alt_r
     roofline["frac_of_nominal_int8_4500"] = tensor["achieved"] / 4500.0
-
-    cpu = None
-    if not args.no_cpu_baseline:
-        dt, nch, nthreads = oracle_sample(cfg, args.cpu_seconds)
-        frac = nch / cfg.nchan
-        cpu = {"value": wl["ops_step"] * frac / dt / 1e12, "unit": "TOPS", "cores": nthreads, "kind": "oracle",
-               "sample": "%d of %d channels (evenly spaced), all %d span(s), full ntime and ninputs; %.1f s" % (
-                   nch, cfg.nchan, cfg.nspans, dt),
-               "samples_per_s": wl["samples_step"] * frac / dt}
+    if same_mix is not None:
+        # what a no-math kernel with the same read : write mix reaches on this box in this run, beside the copy peak
+        roofline["same_mix_peak"] = same_mix["gbs"]
+        roofline["same_mix_frac"] = hbm["achieved"] / same_mix["gbs"]
+        roofline["same_mix_probe"] = same_mix
 
     line = {"metric": METRIC, "value": value, "unit": "TOPS", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
@@ -544,8 +628,9 @@ def main():
                                         "parallelism": "channels sharded, no collective" if world > 1 else "1 gpu",
                                         "algo": args.algo}),
             "samples_per_s": wl["samples_step"] * world / (ms_per_step * 1e-3),
+            "ms_per_step_median": step_ms[len(step_ms) // 2], "ms_per_step_min": step_ms[0],
             "clocks": clocks, "e2e": e2e, "gpu_launches": timed_launches, "roofline": roofline,
-            "cpu_baseline": cpu}
+            "cpu_baseline": cpu, "parity": parity, "sustained": sustained}
     print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()

@@ -105,6 +105,10 @@ int bfXcorrGetMaxSafeNtime(bfXcorr plan, unsigned long long* nt);    /* samples 
 /* Select the kernel (see bfXcorrAlgo).  errors: INVALID_HANDLE, INVALID_ARGUMENT. */
 int bfXcorrSetAlgo(bfXcorr plan, int algo);
 
+/* Name of the kernel (and variant) bfXcorrExecute launches for this plan with the given `accumulate`: a static string,
+ * "" for an invalid handle.  For reports (bench.py's roofline.kernel); the dispatch rule itself lives in the library. */
+const char* bfXcorrGetKernelName(bfXcorr plan, int accumulate);
+
 /* Number of kernels the last bfXcorrExecute on this plan launched (for launch accounting). */
 int bfXcorrGetLaunchCount(bfXcorr plan, int* nlaunch);
 
@@ -135,6 +139,14 @@ int bfXcorrExecuteHost(bfXcorr plan, const void* in_host, void* out_dev, void* o
  *   stream : as bfXcorrExecute; the call only enqueues.
  *   errors : INVALID_HANDLE; INVALID_POINTER (NULL or misaligned); DEVICE_ERROR. */
 int bfXcorrDump(bfXcorr plan, void* acc, void* out, float scale, int zero_acc, void* stream);
+
+/* Measurement aid (the same-mix HBM ceiling): a no-math streaming kernel that moves exactly
+ * the path's algorithmic bytes with coalesced, contiguous accesses -- reads the span once, and writes the visibility
+ * buffer once (accumulate = 0) or reads, increments and rewrites it (accumulate != 0).  It computes nothing of the
+ * method; `out` is left holding meaningless values.  bench.py times it beside bfXcorrExecute and reports the
+ * bandwidth it reaches as roofline.same_mix_peak.
+ *   in, out, stream : as bfXcorrExecute (sizes from the plan).  errors: as bfXcorrExecute. */
+int bfXcorrMemoryProbe(bfXcorr plan, const void* in, void* out, int accumulate, void* stream);
 
 /* Static string for a status code (never NULL). */
 const char* bfXcorrGetStatusString(int status);

@@ -24,11 +24,13 @@ from .binding import (  # noqa: F401
     bfXcorrExecute,
     bfXcorrExecuteHost,
     bfXcorrGetInputBytes,
+    bfXcorrGetKernelName,
     bfXcorrGetLastCudaError,
     bfXcorrGetLaunchCount,
     bfXcorrGetMaxSafeNtime,
     bfXcorrGetOutputBytes,
     bfXcorrGetStatusString,
+    bfXcorrMemoryProbe,
     bfXcorrSetAlgo,
     lib,
 )

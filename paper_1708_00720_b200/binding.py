@@ -36,7 +36,9 @@ SIGNATURES = {
     "bfXcorrGetLastCudaError": (_i, [_vp, _ip]),
     "bfXcorrExecuteHost": (_i, [_vp, _vp, _vp, _vp, _i, _vp]),
     "bfXcorrDump": (_i, [_vp, _vp, _vp, ctypes.c_float, _i, _vp]),
+    "bfXcorrMemoryProbe": (_i, [_vp, _vp, _vp, _i, _vp]),
     "bfXcorrGetStatusString": (ctypes.c_char_p, [_i]),
+    "bfXcorrGetKernelName": (ctypes.c_char_p, [_vp, _i]),
     # include/bfbeamform.h
     "bfBeamformCreate": (_i, [ctypes.POINTER(_vp), _i, _i, _i, _i, _i]),
     "bfBeamformSetWeights": (_i, [_vp, _vp, _vp]),
@@ -103,6 +105,11 @@ def bfXcorrDump(plan: _vp, acc_ptr: int, out_ptr: int, scale: float = 1.0, zero_
            "bfXcorrDump")
 
 
+def bfXcorrMemoryProbe(plan: _vp, in_ptr: int, out_ptr: int, accumulate: bool, stream: int = 0) -> None:
+    """No-math streaming kernel with the path's HBM access mix (measurement aid); `out` is left with meaningless values."""
+    _check(lib().bfXcorrMemoryProbe(plan, _vp(in_ptr), _vp(out_ptr), 1 if accumulate else 0, _vp(stream)), "bfXcorrMemoryProbe")
+
+
 def bfXcorrDestroy(plan: _vp) -> None:
     _check(lib().bfXcorrDestroy(plan), "bfXcorrDestroy")
 
@@ -127,6 +134,10 @@ def bfXcorrGetMaxSafeNtime(plan: _vp) -> int:
 
 def bfXcorrSetAlgo(plan: _vp, algo: int) -> None:
     _check(lib().bfXcorrSetAlgo(plan, algo), "bfXcorrSetAlgo")
+
+
+def bfXcorrGetKernelName(plan: _vp, accumulate: bool) -> str:
+    return lib().bfXcorrGetKernelName(plan, 1 if accumulate else 0).decode()
 
 
 def bfXcorrGetLaunchCount(plan: _vp) -> int:

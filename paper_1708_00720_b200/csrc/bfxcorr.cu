@@ -11,6 +11,7 @@
 #include "../../include/bfxcorr.h"
 #include "xcorr_simt.cuh"
 #include "xcorr_dump.cuh"
+#include "mem_probe.cuh"
 #include "xcorr_few.cuh"
 #include "xcorr_pair.cuh"
 #include "xcorr_pair4.cuh"
@@ -435,6 +436,23 @@ int bfXcorrDump(bfXcorr plan, void* acc, void* out, float scale, int zero_acc, v
     return BF_XCORR_OK;
 }
 
+int bfXcorrMemoryProbe(bfXcorr plan, const void* in, void* out, int accumulate, void* stream)
+{
+    if (!valid(plan)) return BF_XCORR_INVALID_HANDLE;
+    if (!in || !out) return BF_XCORR_INVALID_POINTER;
+    if ((reinterpret_cast<uintptr_t>(in) & 15u) || (reinterpret_cast<uintptr_t>(out) & 15u)) return BF_XCORR_INVALID_POINTER;
+    const long long nin = static_cast<long long>(input_bytes(plan) / 16), nout = static_cast<long long>(output_bytes(plan) / 16);
+    const int grid = 4 * plan->num_sms;
+    plan->last_launch_count = 0;
+    bfx::mem_probe_kernel<<<grid, bfx::MP_THREADS, 0, static_cast<cudaStream_t>(stream)>>>(
+        static_cast<const uint4*>(in), nin, static_cast<uint4*>(out), nout, accumulate ? 1 : 0,
+        reinterpret_cast<unsigned int*>(plan->d_sched + 3));
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(plan, e);
+    plan->last_launch_count = 1;
+    return BF_XCORR_OK;
+}
+
 int bfXcorrDestroy(bfXcorr plan)
 {
     if (!valid(plan)) return BF_XCORR_INVALID_HANDLE;
@@ -486,6 +504,19 @@ int bfXcorrSetAlgo(bfXcorr plan, int algo)
     if (algo != BF_XCORR_ALGO_TCGEN05 && algo != BF_XCORR_ALGO_SIMT) return BF_XCORR_INVALID_ARGUMENT;
     plan->algo = algo;
     return BF_XCORR_OK;
+}
+
+const char* bfXcorrGetKernelName(bfXcorr plan, int accumulate)
+{
+    if (!valid(plan)) return "";
+    if (plan->algo == BF_XCORR_ALGO_SIMT) return "xcorr_simt_kernel";
+    if (!plan->pair) return plan->dtype == BF_XCORR_CI4 ? "xcorr_few_kernel<ci4>" : "xcorr_few_kernel<ci8>";
+    if (plan->dtype == BF_XCORR_CI4) return plan->d_z ? "xcorr_pair4_kernel (S1 ring)" : "xcorr_pair4_kernel (in place)";
+    if (plan->stripe) {
+        if (plan->d_z) return "xcorr_stripe_kernel<ring, staged epilogue>";
+        return accumulate ? "xcorr_stripe_kernel<in place, staged L2-reduce epilogue>" : "xcorr_stripe_kernel<in place, register-direct epilogue>";
+    }
+    return plan->d_z ? "xcorr_pair_kernel (S1 ring)" : "xcorr_pair_kernel (in place)";
 }
 
 int bfXcorrGetLaunchCount(bfXcorr plan, int* nlaunch)
