@@ -15,8 +15,8 @@
  * Data formats:
  *   span `in`     : DEVICE pointer, [ntime][nchan][ninputs] ci4 or ci8, exactly as in include/bfxcorr.h.
  *   weights       : DEVICE pointer, dense [nchan][nbeam][ninputs], input fastest, always 8+8 bit: byte 0 = re,
- *                   byte 1 = im, two's-complement int8.  re may be any code; im must lie in [-127, 127] (symmetric
- *                   quantisation): the kernel holds -im as an int8 operand, and -(-128) does not exist.
+ *                   byte 1 = im, two's-complement int8.  Every code is legal for both parts, -128 included (the plan
+ *                   holds the weights as unsigned bytes with an offset that the kernel takes out again, exactly).
  *   output `out`  : DEVICE pointer, [ntime][nchan][nbeam][2] int32.
  *   Arithmetic    : exact integer.  |b| components are below 2 * ninputs * 128 * 128 <= 2^30 for every legal plan,
  *                   so int32 never wraps.
@@ -40,24 +40,24 @@ typedef struct bfBeamform_impl* bfBeamform; /* opaque plan handle */
 
 /* Create a plan for spans of `ntime` samples x `nchan` channels x `ninputs` inputs of `dtype` and `nbeam` beams.
  *   errors : INVALID_POINTER (plan NULL); INVALID_ARGUMENT (a dimension <= 0); INVALID_DTYPE;
- *            UNSUPPORTED_SHAPE (ninputs * bytes_per_sample not a multiple of 16; ninputs > 32768; nbeam > 128);
+ *            UNSUPPORTED_SHAPE (ninputs * bytes_per_sample not a multiple of 16; ninputs > 32768; nbeam > 127: two
+ *            accumulator columns per beam plus two for the offset sums must fit one 256-column MMA);
  *            UNSUPPORTED_DEVICE; MEM_ALLOC_FAILED; DEVICE_ERROR. */
 int bfBeamformCreate(bfBeamform* plan, int ninputs, int nchan, int ntime, int nbeam, int dtype);
 
-/* Load a weight set.  The weights are re-ordered on the device into the plan's int8 operand layout (one real row
- * (wr, -wi) and one (wi, wr) per beam, matching the order in which the kernel unpacks the voltages) and checked.
- * The call synchronises `stream` before it returns.
+/* Load a weight set.  The weights are re-ordered on the device into the plan's unsigned 8-bit operand layout (one row
+ * (wr + 128, 127 - wi) and one (wi + 128, wr + 128) per beam, matching the order in which the kernel unpacks the
+ * voltages).  The call synchronises `stream` before it returns.
  *   weights : device pointer, [nchan][nbeam][ninputs] ci8, 2-byte aligned.
- *   errors  : INVALID_HANDLE; INVALID_POINTER; INVALID_ARGUMENT (an imaginary part is -128; the plan then holds no
- *             usable weights); DEVICE_ERROR. */
+ *   errors  : INVALID_HANDLE; INVALID_POINTER; DEVICE_ERROR. */
 int bfBeamformSetWeights(bfBeamform plan, const void* weights, void* stream);
 
 /* Beamform one span with the weights loaded last.
  *   in     : device pointer to the span, 16-byte aligned, read only.
  *   out    : device pointer, bfBeamformGetOutputBytes bytes, 8-byte aligned (16 if nbeam is even); overwritten.
  *   stream : a cudaStream_t passed as void*; the call only enqueues.
- *   errors : INVALID_HANDLE; INVALID_POINTER (NULL or misaligned); INVALID_ARGUMENT (no weights loaded);
- *            DEVICE_ERROR. */
+ *   errors : INVALID_HANDLE; INVALID_POINTER (NULL or misaligned); INVALID_ARGUMENT (no weights loaded, or the
+ *            current CUDA device is not the one the plan was created on); DEVICE_ERROR. */
 int bfBeamformExecute(bfBeamform plan, const void* in, void* out, void* stream);
 
 /* Release the plan and its device scratch.  errors: INVALID_HANDLE. */

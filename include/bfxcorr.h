@@ -91,7 +91,8 @@ int bfXcorrCreate(bfXcorr* plan, int ninputs, int nchan, int ntime, int dtype);
  *   out        : device pointer to the visibilities, 16-byte aligned, bfXcorrGetOutputBytes bytes.
  *   accumulate : 0 = overwrite `out` (it need not be initialised); non-zero = out += this span.
  *   stream     : a cudaStream_t passed as void* (NULL = the legacy default stream).
- *   errors     : INVALID_HANDLE; INVALID_POINTER (NULL or misaligned); DEVICE_ERROR (launch failed). */
+ *   errors     : INVALID_HANDLE; INVALID_POINTER (NULL or misaligned); INVALID_ARGUMENT (the current CUDA device is not
+ *                the one the plan was created on); DEVICE_ERROR (launch failed). */
 int bfXcorrExecute(bfXcorr plan, const void* in, void* out, int accumulate, void* stream);
 
 /* Release the plan and its device scratch.  errors: INVALID_HANDLE (NULL). */

@@ -177,18 +177,16 @@ long long xcorr_oracle_dump(int32_t* acc, float* out, long long ncomponents, flo
  *       out[t][c][k] = b            (int32 re, int32 im; sums taken in int64 and truncated to 32 bits)
  *
  * x as above (ci4 or ci8).  Weights w: dense [nchan][nbeam][ninputs], input fastest, always 8+8 bit: byte 0 = re,
- * byte 1 = im, int8.  The code -128 is legal for re; for im it is outside the domain (the quantised weights are
- * symmetric, [-127, 127]) and the routine rejects it (returns -2).
+ * byte 1 = im, int8.  Every code is legal for both parts, -128 included (reading B4: as for the
+ * voltages, reading A6, the extreme code is ordinary input and the result must stay exact).
  * Returns the number of sums that did not fit in int32 (0 for every legal input: 2 * 32768 * 128 * 128 < 2^31
  * holds up to 32768 inputs), -1 on bad arguments. */
 long long xcorr_oracle_beamform(const uint8_t* in, const uint8_t* w, int32_t* out, int ninputs, int nchan,
                                 int ntime, int nbeam, int dtype)
 {
     const long long N = ninputs, C = nchan, T = ntime, K = nbeam;
-    long long nwrap = 0, q;
+    long long nwrap = 0;
     if (!in || !w || !out || N <= 0 || C <= 0 || T <= 0 || K <= 0 || (dtype != 4 && dtype != 8)) return -1;
-    for (q = 0; q < C * K * N; ++q)
-        if ((int8_t)w[2 * q + 1] == -128) return -2;
 #ifdef _OPENMP
 #pragma omp parallel for collapse(2) reduction(+ : nwrap) schedule(static)
 #endif

@@ -138,8 +138,6 @@ def beamform(x: np.ndarray, w: np.ndarray, ninputs: int, nchan: int, ntime: int,
     fn.restype = ctypes.c_longlong
     fn.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p] + [ctypes.c_int] * 5
     nwrap = fn(x.ctypes.data, w.ctypes.data, out.ctypes.data, ninputs, nchan, ntime, nbeam, dtype)
-    if nwrap == -2:
-        raise ValueError("weight imaginary part -128 is outside the domain")
     if nwrap < 0:
         raise ValueError("xcorr_oracle_beamform rejected its arguments")
     return (out, int(nwrap)) if return_nwrap else out

@@ -2,10 +2,15 @@
 //
 // Per channel c it is the dense contraction  b[t][k] = sum_i w[c][k][i] x[t][c][i]  over the INPUT axis, so, unlike
 // the X-engine, the span rows are already the K-major operand: a row x[t][c][0..N) of ci8 samples is, byte for byte,
-// the int8 row a[t][0..2N) with a[2i] = re_i, a[2i+1] = im_i, and the plan holds, per channel, two int8 rows per beam
-//     W[2k  ][2i] =  wr   W[2k  ][2i+1] = -wi          ->  D[t][2k]   = Re b[t][k]
-//     W[2k+1][2i] =  wi   W[2k+1][2i+1] =  wr          ->  D[t][2k+1] = Im b[t][k]
-// (bfBeamformSetWeights; kind::i8 cannot negate an operand, hence the im != -128 domain).  ci4 rows are widened
+// the int8 row a[t][0..2N) with a[2i] = re_i, a[2i+1] = im_i.  Re b needs -wi, kind::i8 cannot negate an operand, and
+// -(-128) is no int8: so the weight operand is UNSIGNED 8-bit (the instruction descriptor gives A and B their own
+// formats) and holds every weight with an offset; per channel, two rows per beam and two rows of selectors:
+//     W[2k  ][2i] = wr + 128   W[2k  ][2i+1] = 127 - wi    ->  D[t][2k]   = Re b[t][k] + 128 Sr[t] + 127 Si[t]
+//     W[2k+1][2i] = wi + 128   W[2k+1][2i+1] = wr + 128    ->  D[t][2k+1] = Im b[t][k] + 128 Sr[t] + 128 Si[t]
+//     W[2K  ][2i] = 1          W[2K  ][2i+1] = 0           ->  D[t][2K]   = Sr[t] = sum_i re_i
+//     W[2K+1][2i] = 0          W[2K+1][2i+1] = 1           ->  D[t][2K+1] = Si[t] = sum_i im_i
+// (bfBeamformSetWeights); the epilogue subtracts the offsets, exactly (int32, wrapping), so every weight code
+// including -128 - 128j is legal (reading B4).  ci4 rows are widened
 // on chip as in xcorr_pair4.cuh: each 32-bit word of 4 samples becomes the 4 re bytes (<< 4) then the 4 im bytes
 // (<< 4), the weight rows are stored in the same grouped order, and the factor 16 is shifted out exactly in the
 // epilogue.  Every sample is used once, so the span is consumed in place: no ring, no relayout.
@@ -79,10 +84,10 @@ __device__ __forceinline__ uint64_t bm_smem_desc(uint32_t saddr)
     return d;
 }
 
-// UMMA instruction descriptor: dense, D = S32, A = B = signed int8, both K-major
+// UMMA instruction descriptor: dense, D = S32, A = signed int8 (voltages), B = UNSIGNED int8 (offset weights), both K-major
 __host__ __device__ constexpr uint32_t bm_instr_desc(int m, int n)
 {
-    return (2u << 4) | (1u << 7) | (1u << 10) | (static_cast<uint32_t>(n >> 3) << 17) | (static_cast<uint32_t>(m >> 4) << 24);
+    return (2u << 4) | (1u << 7) | (0u << 10) | (static_cast<uint32_t>(n >> 3) << 17) | (static_cast<uint32_t>(m >> 4) << 24);
 }
 
 template <bool CI4>
@@ -234,13 +239,19 @@ beamform_kernel(const __grid_constant__ CUtensorMap xmap, const __grid_constant_
             const int t = un.t0 + 32 * wq + static_cast<int>(lane);
             int32_t* const orow = p.out + 2 * ((static_cast<long long>(t) * p.nchan + un.c) * p.nbeam);
             const int nrows = p.ntime - (un.t0 + 32 * wq);   // rows of this warp that exist
+            // this sample's Sr, Si (columns 2 nbeam, 2 nbeam + 1): the offsets carried by every beam column
+            uint32_t sr, si;
+            ptx::tmem_ld_32x32b_x2(tmem_base + (static_cast<uint32_t>(32 * wq) << 16) + 256 * b + 2 * p.nbeam, sr, si);
+            ptx::tmem_ld_wait();
+            const uint32_t off_re = 128u * sr + 127u * si, off_im = 128u * (sr + si);
             for (int col = 0; col < 2 * p.nbeam; col += 32) {
                 uint32_t r[32];
                 ptx::tmem_ld_32x32b_x32(tmem_base + (static_cast<uint32_t>(32 * wq) << 16) + 256 * b + col, r);
                 ptx::tmem_ld_wait();
-                if (CI4) {
 #pragma unroll
-                    for (int j = 0; j < 32; ++j) r[j] = static_cast<uint32_t>(static_cast<int32_t>(r[j]) >> 4);
+                for (int j = 0; j < 32; ++j) {
+                    r[j] -= (j & 1) ? off_im : off_re;   // exact in wrapping int32: the true beam fits (|b| < 2^31)
+                    if (CI4) r[j] = static_cast<uint32_t>(static_cast<int32_t>(r[j]) >> 4);   // x was widened as 16 x
                 }
 #ifdef BFX_BM_NO_STORE
                 if (nrows < -p.ntime) {
@@ -337,12 +348,12 @@ beamform_kernel(const __grid_constant__ CUtensorMap xmap, const __grid_constant_
     if (warp == 2) ptx::tmem_dealloc<1>(tmem_base, 512);
 }
 
-// bfBeamformSetWeights: w[c][k][i] (ci8) -> W[c][n][kk] int8, n = 2k + part of b, kk in the order the loaders write
-// the span bytes (header comment); rows n >= 2 nbeam and columns beyond the inputs are zero.  *bad |= 1 if an
-// imaginary part is -128.
+// bfBeamformSetWeights: w[c][k][i] (ci8) -> W[c][n][kk] uint8, n = 2k + part of b for the beams, n = 2 nbeam, 2 nbeam + 1
+// the selector rows, kk in the order the loaders write the span bytes (header comment); the other rows, and the columns
+// beyond the inputs, are zero (the span reads as zero there too).
 template <bool CI4>
-__global__ void beamform_weights_kernel(const int8_t* __restrict__ w, int8_t* __restrict__ wp, int ninputs, int nchan, int nbeam,
-                                        int nb2, int kp, int* bad)
+__global__ void beamform_weights_kernel(const int8_t* __restrict__ w, uint8_t* __restrict__ wp, int ninputs, int nchan, int nbeam,
+                                        int nb2, int kp)
 {
     const long long total = static_cast<long long>(nchan) * nb2 * kp;
     for (long long q = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x; q < total;
@@ -360,13 +371,16 @@ __global__ void beamform_weights_kernel(const int8_t* __restrict__ w, int8_t* __
             xpart = kk & 1;
         }
         int v = 0;
-        if (k < nbeam && i < ninputs) {
-            const int8_t* s = w + 2 * ((static_cast<long long>(c) * nbeam + k) * ninputs + i);
-            const int wr = s[0], wi = s[1];
-            if (wi == -128) atomicOr(bad, 1);
-            v = bpart == 0 ? (xpart == 0 ? wr : -wi) : (xpart == 0 ? wi : wr);
+        if (i < ninputs) {
+            if (k < nbeam) {
+                const int8_t* s = w + 2 * ((static_cast<long long>(c) * nbeam + k) * ninputs + i);
+                const int wr = s[0], wi = s[1];
+                v = bpart == 0 ? (xpart == 0 ? wr + 128 : 127 - wi) : (xpart == 0 ? wi + 128 : wr + 128);
+            } else if (k == nbeam) {
+                v = bpart == xpart ? 1 : 0;   // row 2 nbeam selects the re components, row 2 nbeam + 1 the im components
+            }
         }
-        wp[q] = static_cast<int8_t>(v);
+        wp[q] = static_cast<uint8_t>(v);
     }
 }
 

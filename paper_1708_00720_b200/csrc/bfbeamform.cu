@@ -30,11 +30,11 @@ constexpr uint32_t kMagic = 0xBFBEA301u;
 struct bfBeamform_impl {
     uint32_t magic;
     int ninputs, nchan, ntime, nbeam, dtype;
+    int device;     // the plan's scratch lives on this device
     int num_sms;
     int last_cuda_error;
     int have_weights;
-    int8_t* d_wp;   // re-ordered weights W[nchan][nb2][kp] int8 (beamform.cuh)
-    int* d_bad;     // set by the re-ordering kernel if an imaginary part is -128
+    uint8_t* d_wp;  // re-ordered, offset weights W[nchan][nb2][kp] uint8 (beamform.cuh)
     int nb2, kp;
     CUtensorMap wmap;
     EncodeTiledFn encode;
@@ -57,7 +57,6 @@ unsigned long long bps(int dtype) { return dtype == BF_XCORR_CI4 ? 1ull : 2ull; 
 void release(bfBeamform p)
 {
     if (p->d_wp) cudaFree(p->d_wp);
-    if (p->d_bad) cudaFree(p->d_bad);
     p->magic = 0;
     delete p;
 }
@@ -73,7 +72,7 @@ int bfBeamformCreate(bfBeamform* plan, int ninputs, int nchan, int ntime, int nb
     if (ninputs <= 0 || nchan <= 0 || ntime <= 0 || nbeam <= 0) return BF_XCORR_INVALID_ARGUMENT;
     if (dtype != BF_XCORR_CI4 && dtype != BF_XCORR_CI8) return BF_XCORR_INVALID_DTYPE;
     if ((static_cast<unsigned long long>(ninputs) * bps(dtype)) % 16ull != 0) return BF_XCORR_UNSUPPORTED_SHAPE;
-    if (ninputs > 32768 || nbeam > 128) return BF_XCORR_UNSUPPORTED_SHAPE;
+    if (ninputs > 32768 || nbeam > 127) return BF_XCORR_UNSUPPORTED_SHAPE;   // 2 nbeam + 2 accumulator columns <= 256
 
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev <= 0) {
@@ -95,6 +94,7 @@ int bfBeamformCreate(bfBeamform* plan, int ninputs, int nchan, int ntime, int nb
     p->ntime = ntime;
     p->nbeam = nbeam;
     p->dtype = dtype;
+    p->device = dev;
     p->num_sms = prop.multiProcessorCount;
 
     void* fn = nullptr;
@@ -114,7 +114,7 @@ int bfBeamformCreate(bfBeamform* plan, int ninputs, int nchan, int ntime, int nb
     q.ntime = ntime;
     q.nbeam = nbeam;
     q.row_in = row_in;
-    q.nb2 = (2 * nbeam + 15) / 16 * 16;
+    q.nb2 = (2 * nbeam + 2 + 15) / 16 * 16;   // two rows per beam + the two selector rows (beamform.cuh)
     q.nks = (row_in + 127) / 128;
     q.ntb = (ntime + bfx::BM_MT - 1) / bfx::BM_MT;
     q.nunits = static_cast<long long>(q.ntb) * nchan;
@@ -127,7 +127,10 @@ int bfBeamformCreate(bfBeamform* plan, int ninputs, int nchan, int ntime, int nb
     int raw = ci4 ? (2u * stage_bytes + 4u * raw_tile + fixed <= static_cast<unsigned>(bfx::BM_SMEM_MAX) ? 4 : 2) : 0;
     int stages = static_cast<int>((bfx::BM_SMEM_MAX - fixed - raw * raw_tile) / stage_bytes);
     if (stages > bfx::BM_MAX_STAGES) stages = bfx::BM_MAX_STAGES;
-    q.stages = stages;  // >= 2 for every nb2 <= 256
+    // ci8: >= 2 for every nb2 <= 256.  ci4 with nb2 > 208 (more than 103 beams): the two widened K tiles of a stage take
+    // 2 * (16 KiB + 128 nb2) bytes and only ONE stage fits beside the raw ring and the staging -- loads, widening and MMA
+    // then run one after the other (exact, but about 2.5 x slower per byte: DESIGN.md section 11)
+    q.stages = stages;
     q.raw_stages = raw;
     p->smem_bytes = static_cast<unsigned>(stages) * stage_bytes + raw * raw_tile + fixed;
     p->encode = reinterpret_cast<EncodeTiledFn>(fn);
@@ -139,7 +142,6 @@ int bfBeamformCreate(bfBeamform* plan, int ninputs, int nchan, int ntime, int nb
 
     const size_t wbytes = static_cast<size_t>(nchan) * q.nb2 * p->kp;
     e = cudaMalloc(reinterpret_cast<void**>(&p->d_wp), wbytes);
-    if (e == cudaSuccess) e = cudaMalloc(reinterpret_cast<void**>(&p->d_bad), sizeof(int));
     if (e == cudaSuccess)
         e = cudaFuncSetAttribute(bfx::beamform_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bfx::BM_SMEM_MAX);
     if (e == cudaSuccess)
@@ -171,24 +173,20 @@ int bfBeamformSetWeights(bfBeamform p, const void* weights, void* stream)
     if (!weights || (reinterpret_cast<uintptr_t>(weights) & 1u)) return BF_XCORR_INVALID_POINTER;
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     p->have_weights = 0;
-    cudaError_t e = cudaMemsetAsync(p->d_bad, 0, sizeof(int), s);
-    if (e != cudaSuccess) return cuda_fail(p, e);
+    cudaError_t e = cudaSuccess;
     const long long total = static_cast<long long>(p->nchan) * p->nb2 * p->kp;
     long long blocks = (total + 255) / 256;
     if (blocks > 32ll * p->num_sms) blocks = 32ll * p->num_sms;
     if (p->dtype == BF_XCORR_CI4)
         bfx::beamform_weights_kernel<true><<<static_cast<unsigned>(blocks), 256, 0, s>>>(
-            static_cast<const int8_t*>(weights), p->d_wp, p->ninputs, p->nchan, p->nbeam, p->nb2, p->kp, p->d_bad);
+            static_cast<const int8_t*>(weights), p->d_wp, p->ninputs, p->nchan, p->nbeam, p->nb2, p->kp);
     else
         bfx::beamform_weights_kernel<false><<<static_cast<unsigned>(blocks), 256, 0, s>>>(
-            static_cast<const int8_t*>(weights), p->d_wp, p->ninputs, p->nchan, p->nbeam, p->nb2, p->kp, p->d_bad);
+            static_cast<const int8_t*>(weights), p->d_wp, p->ninputs, p->nchan, p->nbeam, p->nb2, p->kp);
     e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(p, e);
-    int bad = 0;
-    e = cudaMemcpyAsync(&bad, p->d_bad, sizeof(int), cudaMemcpyDeviceToHost, s);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    e = cudaStreamSynchronize(s);   // the caller's weight buffer may be reused once this call has returned
     if (e != cudaSuccess) return cuda_fail(p, e);
-    if (bad) return BF_XCORR_INVALID_ARGUMENT;
     p->have_weights = 1;
     return BF_XCORR_OK;
 }
@@ -199,6 +197,8 @@ int bfBeamformExecute(bfBeamform p, const void* in, void* out, void* stream)
     if (!in || !out || (reinterpret_cast<uintptr_t>(in) & 15u)) return BF_XCORR_INVALID_POINTER;
     if (reinterpret_cast<uintptr_t>(out) & ((p->nbeam & 1) ? 7u : 15u)) return BF_XCORR_INVALID_POINTER;
     if (!p->have_weights) return BF_XCORR_INVALID_ARGUMENT;
+    int cur = -1;
+    if (cudaGetDevice(&cur) != cudaSuccess || cur != p->device) return BF_XCORR_INVALID_ARGUMENT;   // the plan belongs to another device
     bfx::BmParams q = p->prm;
     q.x = static_cast<const uint8_t*>(in);
     q.out = static_cast<int32_t*>(out);

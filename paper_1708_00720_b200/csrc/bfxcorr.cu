@@ -368,6 +368,8 @@ int bfXcorrExecute(bfXcorr plan, const void* in, void* out, int accumulate, void
     if (!in || !out) return BF_XCORR_INVALID_POINTER;
     if ((reinterpret_cast<uintptr_t>(in) & 15u) || (reinterpret_cast<uintptr_t>(out) & 15u)) return BF_XCORR_INVALID_POINTER;
     cudaStream_t s = static_cast<cudaStream_t>(stream);
+    int cur = -1;
+    if (cudaGetDevice(&cur) != cudaSuccess || cur != plan->device) return BF_XCORR_INVALID_ARGUMENT;   // the plan's scratch lives on another device
     plan->last_launch_count = 0;
     if (plan->algo == BF_XCORR_ALGO_SIMT) return launch_simt(plan, in, out, accumulate, s);
     if (plan->d_z) return launch_tcgen05<false>(plan, in, out, accumulate, s);  // S1 fused: dtype handled by the relayout warps

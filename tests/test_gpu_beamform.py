@@ -35,9 +35,9 @@ def run_beamform(x, w, N, C, T, K, dtype, poison=True):
 def _random_case(rng, N, C, T, K, dtype, extreme=False):
     x = rng.integers(0, 256, size=(T, C, N * (1 if dtype == 4 else 2)), dtype=np.uint8)   # every code, -8 / -128 too
     wr = rng.integers(-128, 128, size=(C, K, N))
-    wi = rng.integers(-127, 128, size=(C, K, N))
+    wi = rng.integers(-128, 128, size=(C, K, N))   # the whole int8 range for both parts (reading B4)
     if extreme:
-        wr[:], wi[:] = -128, 127
+        wr[:], wi[:] = -128, -128 if extreme == "neg" else 127
         x[:] = 0x88 if dtype == 4 else 0x80
     w = np.stack((wr & 0xFF, wi & 0xFF), axis=-1).astype(np.uint8).reshape(C, K, 2 * N)
     return x, w
@@ -51,7 +51,7 @@ SHAPES = [
     (80, 7, 129, 3),      # rows that are no multiple of 128 bytes, odd beam count
     (512, 3, 300, 32),    # station shape: several K stages, ragged tail
     (528, 2, 128, 5),
-    (128, 2, 257, 128),   # maximum beam count (N = 256 columns)
+    (128, 2, 257, 127),   # maximum beam count (2 * 127 + 2 = 256 accumulator columns)
     (256, 170, 64, 4),    # more units than SMs with a single short sample block
 ]
 
@@ -69,14 +69,17 @@ def test_matches_oracle(shape, dtype):
     np.testing.assert_array_equal(got, exp)
 
 
+@pytest.mark.parametrize("extreme", ["neg", "mixed"])
 @pytest.mark.parametrize("dtype", [4, 8])
-def test_extreme_codes(dtype):
+def test_extreme_codes(dtype, extreme):
+    """Every sample at the most negative code and every weight -128 - 128j ("neg") or -128 + 127j ("mixed")."""
     N, C, T, K = 512, 2, 140, 8
-    x, w = _random_case(np.random.default_rng(0), N, C, T, K, dtype, extreme=True)
+    x, w = _random_case(np.random.default_rng(0), N, C, T, K, dtype, extreme=extreme)
     np.testing.assert_array_equal(run_beamform(x, w, N, C, T, K, dtype), oracle.beamform(x, w, N, C, T, K, dtype))
 
 
-def test_weight_domain_is_checked():
+def test_no_weights_and_limits():
+    """Execute without weights is refused; every weight code (-128 in either part) is accepted; 128 beams are not."""
     N, C, T, K = 16, 1, 8, 1
     plan = bfx.bfBeamformCreate(N, C, T, K, 8)
     try:
@@ -86,20 +89,19 @@ def test_weight_domain_is_checked():
         with pytest.raises(bfx.BfXcorrError) as e:     # no weights yet
             bfx.bfBeamformExecute(plan, x.data_ptr(), out.data_ptr(), 0)
         assert e.value.status == 3
-        w[5] = 0x80                                    # an imaginary part of -128
-        with pytest.raises(bfx.BfXcorrError) as e:
-            bfx.bfBeamformSetWeights(plan, w.data_ptr(), 0)
-        assert e.value.status == 3
-        w[5] = 0x81
-        w[4] = 0x80                                    # a real part of -128 is legal
+        w[4] = 0x80
+        w[5] = 0x80                                    # -128 - 128j
         bfx.bfBeamformSetWeights(plan, w.data_ptr(), 0)
         bfx.bfBeamformExecute(plan, x.data_ptr(), out.data_ptr(), 0)
         torch.cuda.synchronize()
     finally:
         bfx.bfBeamformDestroy(plan)
+    with pytest.raises(bfx.BfXcorrError) as e:
+        bfx.bfBeamformCreate(N, C, T, 128, 8)
+    assert e.value.status == 5
 
 
-@pytest.mark.parametrize("name,nbeam", [("cfg2", 32), ("cfg3", 16), ("cfg4", 16), ("cfg5", 8), ("cfg2", 128), ("cfg2", 7)])
+@pytest.mark.parametrize("name,nbeam", [("cfg2", 32), ("cfg3", 16), ("cfg4", 16), ("cfg5", 8), ("cfg2", 127), ("cfg2", 7)])
 def test_full_config_sampled_channels(name, nbeam):
     """BASELINE.json's station-shaped spans at full size, in the launch configuration bench.py times: sampled
     channels (all samples, all beams) against the oracle."""

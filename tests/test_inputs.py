@@ -98,3 +98,15 @@ def test_device_generation_matches_host():
         if cfg.tone_channels:
             cfg = small(cfg, tone_channels=(191,))
         assert torch.equal(generate_span(cfg, 1), generate_span(cfg, 1, device="cuda").cpu())
+
+
+def test_weights_cover_the_whole_int8_range():
+    """generate_weights draws every code, -128 included, for both parts (reading B4)."""
+    from xcorr_inputs import generate_weights
+    w = generate_weights(7, 4, 8, 256).view(torch.int8).reshape(4, 8, 256, 2)
+    for part in (0, 1):
+        v = w[..., part]
+        assert int(v.min()) == -128 and int(v.max()) == 127
+        assert abs(float(v.float().mean())) < 3.0
+    sub = generate_weights(7, 4, 8, 256, channels=[2])
+    assert torch.equal(sub[0], generate_weights(7, 4, 8, 256)[2])

@@ -77,7 +77,7 @@ def test_numpy_complex_matmul(dtype):
     T, C, N, K = 7, 3, 10, 4
     xr, xi = _rand(rng, dtype, (T, C, N))
     wr = rng.integers(-128, 128, size=(C, K, N))
-    wi = rng.integers(-127, 128, size=(C, K, N))
+    wi = rng.integers(-128, 128, size=(C, K, N))
     b = oracle.beamform(pack(dtype, xr, xi), _w(wr, wi), N, C, T, K, dtype)
     xc = xr + 1j * xi
     wc = wr + 1j * wi
@@ -120,20 +120,26 @@ def test_beam_power_equals_the_quadratic_form_of_the_visibilities():
         assert int(round(q.real)) == int((b[:, 0, k, 0] ** 2 + b[:, 0, k, 1] ** 2).sum())
 
 
-def test_extreme_codes_and_domain():
+def test_extreme_codes_whole_weight_range():
     # x = -128 - 128i on 3 inputs, w = -128 + 127i: (-128)(-128) - 127(-128) = 32640; (-128)(-128) + 127(-128) = 128
     x = pack(8, np.full((1, 1, 3), -128), np.full((1, 1, 3), -128))
     b, nwrap = oracle.beamform(x, _w(np.full((1, 1, 3), -128), np.full((1, 1, 3), 127)), 3, 1, 1, 1, 8,
                                return_nwrap=True)
     assert b[0, 0, 0].tolist() == [3 * 32640, 3 * 128] and nwrap == 0
-    with pytest.raises(ValueError):
-        oracle.beamform(x, _w(np.zeros((1, 1, 3)), np.full((1, 1, 3), -128)), 3, 1, 1, 1, 8)
+    # every weight code is legal (reading B4).  w = -128 - 128i on the same x, worked by hand:
+    # (-128 - 128i)(-128 - 128i) = 128^2 (1 + i)^2 = 32768 i   ->   re 0, im 32768 per input
+    b = oracle.beamform(x, _w(np.full((1, 1, 3), -128), np.full((1, 1, 3), -128)), 3, 1, 1, 1, 8)
+    assert b[0, 0, 0].tolist() == [0, 3 * 32768]
+    # w = 0 - 128i, x = 1 + 0i: -128 i;  x = 0 + 1i: (-128 i)(i) = +128
+    b = oracle.beamform(pack(8, np.array([[[1, 0]]]), np.array([[[0, 1]]])),
+                        _w(np.zeros((1, 1, 2)), np.full((1, 1, 2), -128)), 2, 1, 1, 1, 8)
+    assert b[0, 0, 0].tolist() == [128, -128]
 
 
 def test_ci4_equals_ci8_on_the_same_values():
     rng = np.random.default_rng(8)
     T, C, N, K = 4, 2, 16, 3
     xr, xi = _rand(rng, 4, (T, C, N))
-    w = _w(rng.integers(-127, 128, size=(C, K, N)), rng.integers(-127, 128, size=(C, K, N)))
+    w = _w(rng.integers(-128, 128, size=(C, K, N)), rng.integers(-128, 128, size=(C, K, N)))
     assert np.array_equal(oracle.beamform(pack(4, xr, xi), w, N, C, T, K, 4),
                           oracle.beamform(pack(8, xr, xi), w, N, C, T, K, 8))

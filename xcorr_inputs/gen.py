@@ -204,11 +204,11 @@ def generate_channel_slab(cfg: XcorrConfig, span: int, channels: Sequence[int],
 def generate_weights(seed: int, nchan: int, nbeam: int, ninputs: int, channels: Optional[Sequence[int]] = None,
                      device="cpu") -> torch.Tensor:
     """Beamformer weights, ci8 [nchan][nbeam][2 * ninputs] uint8 (byte 0 = re, byte 1 = im), each component a seeded
-    uniform integer in [-127, 127] -- the range of symmetric int8 quantisation; they stand in for quantised steering
-    phasors.  `channels` selects rows of the same draw."""
+    uniform integer over the whole int8 range [-128, 127]; they stand in for quantised steering phasors (SURVEY.md
+    section 8(f) N1).  `channels` selects rows of the same draw."""
     cs = list(range(nchan)) if channels is None else list(channels)
     c = torch.tensor(cs, dtype=torch.int64, device=device).view(-1, 1, 1)
     k = torch.arange(nbeam, dtype=torch.int64, device=device).view(1, -1, 1)
     j = torch.arange(2 * ninputs, dtype=torch.int64, device=device).view(1, 1, -1)
     r = _uniform32(seed ^ 0x5EED0BEA, (c * nbeam + k) * (2 * ninputs) + j)
-    return ((torch.remainder(r, 255) - 127) & 0xFF).to(torch.uint8)
+    return (r & 0xFF).to(torch.uint8)   # 256 equally likely codes = uniform over [-128, 127] in two's complement
