@@ -35,7 +35,13 @@
  * the plan's scheduler words, S1 ring and flags): enqueue them on one stream, or order streams with events.
  * Results are deterministic (integer sums).
  *
- * Errors: every entry point returns a bfXcorrStatus (0 = OK); nothing aborts or throws across the ABI.
+ * Errors: every entry point returns a bfXcorrStatus (0 = OK); no host code aborts or throws across the ABI.
+ * Device side, every wait of the kernels (mbarriers, flags between CTAs) is BOUNDED: should one not complete within
+ * a few seconds -- which only a defect of the library or a corrupted plan can cause, never the data -- the kernel
+ * executes a trap instead of hanging the GPU.  The caller then sees what any faulting kernel produces: the next
+ * synchronising CUDA call on that stream returns cudaErrorLaunchFailure, the error is sticky (the CUDA context is
+ * lost and must be torn down with the process or cudaDeviceReset), and every later call into this library that
+ * touches the device returns BF_XCORR_DEVICE_ERROR.  The contents of `out` are then undefined.
  * There is NO CPU fallback: without a compute-capability-10.x device bfXcorrCreate returns
  * BF_XCORR_UNSUPPORTED_DEVICE.
  */

@@ -253,11 +253,7 @@ beamform_kernel(const __grid_constant__ CUtensorMap xmap, const __grid_constant_
                     r[j] -= (j & 1) ? off_im : off_re;   // exact in wrapping int32: the true beam fits (|b| < 2^31)
                     if (CI4) r[j] = static_cast<uint32_t>(static_cast<int32_t>(r[j]) >> 4);   // x was widened as 16 x
                 }
-#ifdef BFX_BM_NO_STORE
-                if (nrows < -p.ntime) {
-#else
                 {
-#endif
                     if (vec4) {
                         // through shared memory so that eight lanes write one row's 128 contiguous bytes
                         const uint32_t srow = stg_warp + lane * BM_STG_PITCH;

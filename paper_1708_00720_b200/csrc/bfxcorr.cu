@@ -79,6 +79,7 @@ struct bfXcorr_impl {
     cudaStream_t s_h2d, s_d2h;
     cudaEvent_t ev_h2d[2], ev_comp[2], ev_d2h;
     unsigned long long host_calls;
+    bool host_ready;   // staging buffers, copy streams and events all exist
 };
 
 namespace {
@@ -238,6 +239,26 @@ int launch_tcgen05(bfXcorr p, const void* in, void* out, int accumulate, cudaStr
     return BF_XCORR_OK;
 }
 
+// bfXcorrExecuteHost's staging state: released as a whole (also after a partial set-up), pointers nulled
+void release_host_state(bfXcorr plan)
+{
+    for (int b = 0; b < 2; ++b) {
+        if (plan->d_stage_in[b]) cudaFree(plan->d_stage_in[b]);
+        if (plan->ev_h2d[b]) cudaEventDestroy(plan->ev_h2d[b]);
+        if (plan->ev_comp[b]) cudaEventDestroy(plan->ev_comp[b]);
+        plan->d_stage_in[b] = nullptr;
+        plan->ev_h2d[b] = nullptr;
+        plan->ev_comp[b] = nullptr;
+    }
+    if (plan->ev_d2h) cudaEventDestroy(plan->ev_d2h);
+    if (plan->s_h2d) cudaStreamDestroy(plan->s_h2d);
+    if (plan->s_d2h) cudaStreamDestroy(plan->s_d2h);
+    plan->ev_d2h = nullptr;
+    plan->s_h2d = nullptr;
+    plan->s_d2h = nullptr;
+    plan->host_ready = false;
+}
+
 int launch_simt(bfXcorr p, const void* in, void* out, int accumulate, cudaStream_t stream)
 {
     const int nb = (p->ninputs + bfx::SIMT_TILE - 1) / bfx::SIMT_TILE;
@@ -383,7 +404,8 @@ int bfXcorrExecuteHost(bfXcorr plan, const void* in_host, void* out_dev, void* o
     if (!in_host || !out_dev) return BF_XCORR_INVALID_POINTER;
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     cudaError_t e = cudaSuccess;
-    if (!plan->s_h2d) {
+    if (!plan->host_ready) {
+        // first call (or a retry after a failed set-up): everything or nothing, so that a failure can be retried
         e = cudaStreamCreateWithFlags(&plan->s_h2d, cudaStreamNonBlocking);
         if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&plan->s_d2h, cudaStreamNonBlocking);
         for (int b = 0; b < 2 && e == cudaSuccess; ++b) {
@@ -392,7 +414,12 @@ int bfXcorrExecuteHost(bfXcorr plan, const void* in_host, void* out_dev, void* o
             if (e == cudaSuccess) e = cudaEventCreateWithFlags(&plan->ev_comp[b], cudaEventDisableTiming);
         }
         if (e == cudaSuccess) e = cudaEventCreateWithFlags(&plan->ev_d2h, cudaEventDisableTiming);
-        if (e != cudaSuccess) return cuda_fail(plan, e);
+        if (e != cudaSuccess) {
+            release_host_state(plan);
+            return cuda_fail(plan, e);
+        }
+        plan->host_ready = true;
+        plan->host_calls = 0;
     }
     const int b = static_cast<int>(plan->host_calls & 1);
     // span -> staging[b] on the copy stream, once the contraction that last read staging[b] (two calls ago) is done
@@ -459,14 +486,7 @@ int bfXcorrDestroy(bfXcorr plan)
 {
     if (!valid(plan)) return BF_XCORR_INVALID_HANDLE;
     if (plan->d_sched) cudaFree(plan->d_sched);
-    for (int b = 0; b < 2; ++b) {
-        if (plan->d_stage_in[b]) cudaFree(plan->d_stage_in[b]);
-        if (plan->ev_h2d[b]) cudaEventDestroy(plan->ev_h2d[b]);
-        if (plan->ev_comp[b]) cudaEventDestroy(plan->ev_comp[b]);
-    }
-    if (plan->ev_d2h) cudaEventDestroy(plan->ev_d2h);
-    if (plan->s_h2d) cudaStreamDestroy(plan->s_h2d);
-    if (plan->s_d2h) cudaStreamDestroy(plan->s_d2h);
+    release_host_state(plan);
     if (plan->d_z) cudaFree(plan->d_z);
     if (plan->d_flags) cudaFree(plan->d_flags);
     plan->magic = 0;

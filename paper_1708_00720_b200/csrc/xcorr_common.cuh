@@ -25,9 +25,6 @@ namespace bfx {
 
 // ---- tile geometry ----------------------------------------------------------------------------
 // L2 eviction hints (A/B measured, profiles/round1.md): ring slabs evict_last, span reads and visibility writes evict_first
-#ifndef BFX_NO_L2_HINTS
-#define BFX_L2_HINTS 1
-#endif
 #ifndef BFX_KT
 #define BFX_KT 128
 #endif
@@ -68,9 +65,6 @@ struct TcParams {
 #endif
 #ifndef BFX_RL_SLEEP
 #define BFX_RL_SLEEP 500
-#endif
-#ifndef BFX_RL_FENCE
-#define BFX_RL_FENCE 0
 #endif
 constexpr int RL_ROWS = BFX_RL_ROWS;      // samples per relayout unit (4 rounds of 16 loads per lane, one release per unit)
 constexpr int RL_WARPS = 8;      // relayout warps per CTA
@@ -162,16 +156,6 @@ __device__ __forceinline__ void tc_epilogue_chunk(const TcParams& p, uint32_t la
     // chunk with a single buffer: PENDING = 0) must be done with it
     if (lane < 16) ptx::bulk_wait_read<PENDING>();
     __syncwarp();
-#ifdef BFX_PROBE_NO_EPI
-    if (release_bar) {
-        ptx::tc_fence_before();
-        __syncwarp();
-        if (lane == 0) {
-            if (REMOTE_RELEASE) ptx::mbar_arrive_cluster_addr(release_bar); else ptx::mbar_arrive(release_bar);
-        }
-    }
-    return;
-#endif
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
         uint32_t g[32];
@@ -198,9 +182,6 @@ __device__ __forceinline__ void tc_epilogue_chunk(const TcParams& p, uint32_t la
         }
     }
     __syncwarp();
-#ifdef BFX_PROBE_NO_STORE
-    return;
-#endif
     // (Coalesced st.global / red from the staging rows instead of bulk copies was measured slower: 2.38 / 3.10 vs
     // 2.27 / 2.42 ms on cfg3, profiles/round1.md.)
     ptx::fence_proxy_async_smem();  // staging writes -> visible to the bulk-copy engine
@@ -223,14 +204,9 @@ __device__ __forceinline__ void tc_epilogue_chunk(const TcParams& p, uint32_t la
                 if (p.accumulate) ptx::red_add_global_v2(g0, v); else ptx::st_global_v2(g0, v);
             }
             if (nbulk > 0) {
-#ifdef BFX_L2_HINTS
                 // the visibilities stream through the L2 once per span: let them go first, the S1 ring should stay
                 if (p.accumulate) ptx::bulk_reduce_add_s32_hint(g0 + 2 * head, s0 + 8 * head, 8u * nbulk, ptx::policy_evict_first());
                 else ptx::bulk_store_hint(g0 + 2 * head, s0 + 8 * head, 8u * nbulk, ptx::policy_evict_first());
-#else
-                if (p.accumulate) ptx::bulk_reduce_add_s32(g0 + 2 * head, s0 + 8 * head, 8u * nbulk);
-                else ptx::bulk_store(g0 + 2 * head, s0 + 8 * head, 8u * nbulk);
-#endif
             }
             if (head + nbulk < n) {
                 int2 v;
@@ -343,9 +319,6 @@ __device__ __forceinline__ void tc_prefetch_old(const TcParams& p, uint32_t lane
 // Shared by the 1-CTA and the CTA-pair kernels; run by whole warps.
 __device__ __forceinline__ void tc_relayout_role(const TcParams& p, uint32_t lane)
 {
-#ifdef BFX_PROBE_NO_RL
-    return;
-#endif
     // ===================== relayout warps (S1: unpack-and-transpose, span -> ring z) =====================
     // A unit = rl_rows samples x one 1 KiB piece of the (t, c) row of channel cc: read with coalesced 16-byte
     // loads (each span byte exactly once per launch) and written with 16-byte stores to the channel's slab: ci8
@@ -354,7 +327,6 @@ __device__ __forceinline__ void tc_relayout_role(const TcParams& p, uint32_t lan
     const long long src_pitch = static_cast<long long>(p.nchan) * p.row_in;
     const int row_out = p.rl_row_out;  // bytes of one (t, c) row in the ring: 2 N (int8 pairs) or N (packed ci4)
     auto do_unit = [&](int cc, int u) {
-#ifndef BFX_PROBE_RL_ONLY
         if (cc >= p.ring_w) {
             // the slab is still owned by channel cc - ring_w until all of its tiles have loaded their operands
             if (lane == 0) {
@@ -367,7 +339,6 @@ __device__ __forceinline__ void tc_relayout_role(const TcParams& p, uint32_t lan
             }
             __syncwarp();
         }
-#endif
         const int t0 = (u / p.rl_nx) * p.rl_rows;
         const int xb0 = (u % p.rl_nx) * RL_XBYTES;
         const int nt = min(p.rl_rows, p.ntime - t0);
@@ -396,7 +367,6 @@ __device__ __forceinline__ void tc_relayout_role(const TcParams& p, uint32_t lan
         }
         // publish: every lane's stores are ordered before lane 0's release by the warp barrier (the release is
         // cumulative), and made visible to the TMA (async proxy) readers by the proxy fence
-        if (BFX_RL_FENCE) __threadfence();
         ptx::fence_proxy_async_global();
         __syncwarp();
         if (lane == 0) ptx::red_release_add_u64(p.ready + cc, 1ull);

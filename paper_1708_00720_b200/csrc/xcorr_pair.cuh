@@ -91,16 +91,6 @@ struct PrRing {
         long long w = 0;
         if (!WARP || lane == 0)
             asm volatile("ld.shared.s64 %0, [%1];" : "=l"(w) : "r"(ring_base + 8 * slot) : "memory");
-#ifdef BFX_RING_DEBUG
-        // probe build: the publisher tags the index with its iteration number (bits 48..62)
-        if ((!WARP || lane == 0) && w >= 0) {
-            const uint32_t tag = static_cast<uint32_t>(w >> 48);
-            if (tag != (n & 0x3FFFu))
-                printf("ring: warp %d rank %u iteration %u read tag %u (w %lld)\n", static_cast<int>(threadIdx.x >> 5),
-                       ptx::cluster_ctarank(), n, tag, w & 0xFFFFFFFFFFFFll);
-            w &= 0xFFFFFFFFFFFFll;
-        }
-#endif
         if (WARP) w = __shfl_sync(0xffffffffu, w, 0);
         if (!WARP || lane == 0) {
 #if BFX_RING_ARRIVE == 2
@@ -180,9 +170,7 @@ xcorr_pair_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
         // ===================== TMA producer (+ tile scheduler in the leader) =====================
         uint32_t stage = 0, phase = 0;
         int ready_chan = -1;
-#ifdef BFX_L2_HINTS
         const uint64_t pol_last = ptx::policy_evict_last();  // ring slabs are re-read by every tile of the channel
-#endif
         // the leader draws tile n + 1 from the global counter before it loads tile n: the atomic's round trip
         // (and everything the other roles do on receiving an index) overlaps the loads of the current tile
         unsigned long long w_next = 0;
@@ -215,12 +203,10 @@ xcorr_pair_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
                 // the relayout warps (of any CTA) must have written all of z[c]; their generic-proxy stores are
                 // then ordered before our TMA (async proxy) reads
                 if (lane == 0) {
-#ifndef BFX_PROBE_NO_RL
                     const unsigned long long want = p.epoch * static_cast<unsigned long long>(p.rl_units);
                     uint32_t spins = 0;
                     while (ptx::ld_acquire_u64(p.ready + c) < want)
                         if (++spins > (1u << 26)) __trap();
-#endif
                     ptx::fence_proxy_async_global();
                 }
                 __syncwarp();
@@ -234,21 +220,12 @@ xcorr_pair_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
             for (int kb = 0; kb < nkb; ++kb) {
                 ptx::mbar_wait(bar_empty + 8 * stage, phase ^ 1);
                 if (lane == 0) {
-#ifdef BFX_PROBE_NO_TMA
-                    if (leader) ptx::mbar_arrive(bar_full + 8 * stage);
-#else
                     if (leader) ptx::mbar_expect_tx(bar_full + 8 * stage, 2 * cta_bytes);  // both CTAs' boxes
                     const uint32_t dst = op_base + stage * PR_STAGE_BYTES;
                     const uint32_t fullb = lead_full + 8 * stage;
                     const int t0 = kb * TC_KT;
-#ifdef BFX_L2_HINTS
                     ptx::tma_load_3d_cg2_hint(dst, &tmap, fullb, xa, cs, t0, pol_last);
                     if (!diag) ptx::tma_load_3d_cg2_hint(dst + TC_BOX_BYTES, &tmap, fullb, xb, cs, t0, pol_last);
-#else
-                    ptx::tma_load_3d_cg2(dst, &tmap, fullb, xa, cs, t0);
-                    if (!diag) ptx::tma_load_3d_cg2(dst + TC_BOX_BYTES, &tmap, fullb, xb, cs, t0);
-#endif
-#endif
                 }
                 __syncwarp();
                 if (++stage == S) { stage = 0; phase ^= 1; }
@@ -277,10 +254,8 @@ xcorr_pair_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
                     const int trem = p.ntime - kb * TC_KT;
                     const int nk = trem >= TC_KT ? TC_KT / 32 : (trem + 31) / 32;
                     if (lane == 0) {
-#ifndef BFX_PROBE_NO_MMA
                         for (int k = 0; k < nk; ++k)
                             ptx::mma_i8<2>(d_tmem, adesc + 256u * k, bdesc + 256u * k, idesc, (kb | k) != 0 ? 1u : 0u);
-#endif
                         ptx::mma_commit_cg2(bar_empty + 8 * stage, 3);
                     }
                     __syncwarp();
@@ -313,7 +288,6 @@ xcorr_pair_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
             int nchunk = (i0 + 15 - j0) / TC_CJ + 1;
             nchunk = nchunk > 2 ? 2 : nchunk;
             int32_t* const out_c = p.out + 2 * (static_cast<long long>(c) * nbl);
-#ifndef BFX_NO_OUT_PREFETCH
             if (p.accumulate && lane < 16) {
                 // the L2 reduce-adds of this tile will want the old visibilities resident: start pulling this warp's
                 // row segments in now, while the tile is still being contracted
@@ -326,7 +300,6 @@ xcorr_pair_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
                     ptx::bulk_prefetch_l2(out_c + 2 * ea, static_cast<uint32_t>(8 * (eb - ea)));
                 }
             }
-#endif
             ptx::mbar_wait(bar_tfull + 8 * buf, bphase);
             ptx::tc_fence_after();
             for (int jc = 0; jc < nchunk; ++jc, ++nchunks_done) {

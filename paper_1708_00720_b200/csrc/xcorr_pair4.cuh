@@ -50,16 +50,12 @@ __device__ __forceinline__ void p4_tma_load_hint(uint32_t dst, const CUtensorMap
 template <int N>
 __device__ __forceinline__ void p4_regs_inc()
 {
-#ifndef BFX_P4_NO_SETMAXNREG
     asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N));
-#endif
 }
 template <int N>
 __device__ __forceinline__ void p4_regs_dec()
 {
-#ifndef BFX_P4_NO_SETMAXNREG
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N));
-#endif
 }
 
 __global__ void __launch_bounds__(P4_THREADS, 1)
@@ -145,14 +141,9 @@ xcorr_pair4_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
                 if (w >= p.ntiles) w = -1;
                 if (lane == 0) {
                     if (w >= 0) w_next = atomicAdd(p.sched, 1ull);
-#ifdef BFX_RING_DEBUG
-                    const long long wt = w >= 0 ? (w | (static_cast<long long>(n & 0x3FFFu) << 48)) : w;
-#else
-                    const long long wt = w;
-#endif
-                    asm volatile("st.shared.s64 [%0], %1;" ::"r"(ring_base + 8 * slot), "l"(wt) : "memory");
+                    asm volatile("st.shared.s64 [%0], %1;" ::"r"(ring_base + 8 * slot), "l"(w) : "memory");
                     ptx::mbar_arrive(bar_sfull + 8 * slot);
-                    asm volatile("st.shared::cluster.s64 [%0], %1;" ::"r"(ptx::mapa(ring_base + 8 * slot, 1)), "l"(wt) : "memory");
+                    asm volatile("st.shared::cluster.s64 [%0], %1;" ::"r"(ptx::mapa(ring_base + 8 * slot, 1)), "l"(w) : "memory");
                     ptx::mbar_arrive_cluster(bar_sfull + 8 * slot, 1);
                 }
                 w_next = __shfl_sync(0xffffffffu, w_next, 0);
@@ -260,7 +251,6 @@ xcorr_pair4_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
             int nchunk = (i0 + 15 - j0) / TC_CJ + 1;   // 64-column chunks that reach the diagonal or lie below it
             nchunk = nchunk > 2 ? 2 : nchunk;
             int32_t* const out_c = p.out + 2 * (static_cast<long long>(tl.c) * nbl);
-#ifndef BFX_P4_NO_ACC_PREFETCH
             if (p.accumulate && lane < 16) {
                 // the L2 reduce-adds of this tile will want the old visibilities resident
                 const int i_own = i0 + static_cast<int>(lane);
@@ -272,7 +262,6 @@ xcorr_pair4_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
                     ptx::bulk_prefetch_l2(out_c + 2 * ea, static_cast<uint32_t>(8 * (eb - ea)));
                 }
             }
-#endif
             ptx::mbar_wait(bar_tfull + 8 * buf, bphase);
             ptx::tc_fence_after();
             for (int jc = 0; jc < nchunk; ++jc) {
