@@ -367,7 +367,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", default="cfg3", help="cfg1..cfg5 (BASELINE.json configs[0..4])")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--algo", default="tcgen05", choices=["tcgen05", "simt"])
+    ap.add_argument("--algo", default="tcgen05", choices=["tcgen05", "simt", "gauss3"],
+                    help="tcgen05: the product path; simt: the CUDA-core cross-check kernel; gauss3: the three-multiplication ci4 variant")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
@@ -422,7 +423,7 @@ def main():
 
     wl = workload_numbers(cfg)
     peaks = load_peaks()
-    algo = bfx.BF_XCORR_ALGO_TCGEN05 if args.algo == "tcgen05" else bfx.BF_XCORR_ALGO_SIMT
+    algo = {"tcgen05": bfx.BF_XCORR_ALGO_TCGEN05, "simt": bfx.BF_XCORR_ALGO_SIMT, "gauss3": bfx.BF_XCORR_ALGO_TCGEN05_GAUSS3}[args.algo]
 
     # ---- synthetic spans, resident in HBM (every rank holds one full per-GPU workload: a channel shard)
     spans = [generate_span(cfg, s, device=dev) for s in range(cfg.nspans)]

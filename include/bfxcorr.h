@@ -76,10 +76,14 @@ typedef enum bfXcorrStatus_ {
  * lower-triangle tile scheduler, span-accumulate epilogue (CTA pairs above 64 inputs -- with a resident A block per
  * stripe of tiles for ci8 spans of at most 1024 samples --, four channels per CTA up to 64 inputs: DESIGN.md section 5).  SIMT is a plain CUDA-core kernel kept as
  * an on-device cross-check of the tensor path at sizes the CPU oracle cannot reach; it is never
- * selected implicitly. */
+ * selected implicitly.  TCGEN05_GAUSS3 (ci4 plans only) forms the complex product from THREE real tensor-core products
+ * instead of four -- (a+b)c, a(c+d), b(c-d) on operands that fit int8 only because the samples are 4-bit (SURVEY.md
+ * section 8(f) N3; PAPER.md:555 works on the 4+4-bit samples directly): same result bit for bit, 3/4 of the
+ * multiply-accumulates, but measured slower than the default on B200 (profiles/round2.md), so never selected implicitly. */
 typedef enum bfXcorrAlgo_ {
     BF_XCORR_ALGO_TCGEN05 = 0,
-    BF_XCORR_ALGO_SIMT = 1
+    BF_XCORR_ALGO_SIMT = 1,
+    BF_XCORR_ALGO_TCGEN05_GAUSS3 = 2
 } bfXcorrAlgo;
 
 /* Create a plan for spans of exactly `ntime` samples x `nchan` channels x `ninputs` inputs of `dtype`
@@ -109,7 +113,8 @@ int bfXcorrGetInputBytes(bfXcorr plan, unsigned long long* nbytes);  /* ntime*nc
 int bfXcorrGetOutputBytes(bfXcorr plan, unsigned long long* nbytes); /* nchan*ninputs*(ninputs+1)/2*8 */
 int bfXcorrGetMaxSafeNtime(bfXcorr plan, unsigned long long* nt);    /* samples before int32 may wrap */
 
-/* Select the kernel (see bfXcorrAlgo).  errors: INVALID_HANDLE, INVALID_ARGUMENT. */
+/* Select the kernel (see bfXcorrAlgo).  errors: INVALID_HANDLE, INVALID_ARGUMENT (unknown algorithm; GAUSS3 on a ci8
+ * plan), UNSUPPORTED_SHAPE, DEVICE_ERROR. */
 int bfXcorrSetAlgo(bfXcorr plan, int algo);
 
 /* Name of the kernel (and variant) bfXcorrExecute launches for this plan with the given `accumulate`: a static string,

@@ -5,6 +5,7 @@ include/bfxcorr.h and include/bfbeamform.h (built from csrc/ into libbfxcorr.so)
 from .binding import (  # noqa: F401
     BF_XCORR_ALGO_SIMT,
     BF_XCORR_ALGO_TCGEN05,
+    BF_XCORR_ALGO_TCGEN05_GAUSS3,
     BF_XCORR_CI4,
     BF_XCORR_CI8,
     BF_XCORR_OK,

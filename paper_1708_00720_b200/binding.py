@@ -17,6 +17,7 @@ BF_XCORR_CI8 = 8
 BF_XCORR_OK = 0
 BF_XCORR_ALGO_TCGEN05 = 0
 BF_XCORR_ALGO_SIMT = 1
+BF_XCORR_ALGO_TCGEN05_GAUSS3 = 2
 
 _vp = ctypes.c_void_p
 _i = ctypes.c_int

@@ -16,6 +16,7 @@
 #include "xcorr_pair.cuh"
 #include "xcorr_pair4.cuh"
 #include "xcorr_stripe.cuh"
+#include "xcorr_gauss4.cuh"
 #include "xcorr_common.cuh"
 
 namespace {
@@ -239,6 +240,32 @@ int launch_tcgen05(bfXcorr p, const void* in, void* out, int accumulate, cudaStr
     return BF_XCORR_OK;
 }
 
+// xcorr_gauss4.cuh: ci4 spans with the three-multiplication complex product, one CTA per 128 x 128-input tile, in place
+int launch_gauss4(bfXcorr p, const void* in, void* out, int accumulate, cudaStream_t stream)
+{
+    CUtensorMap tmap;
+    const int st = encode_map(p, &tmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, direct_source(p, in), 1, 128u, CU_TENSOR_MAP_SWIZZLE_NONE,
+                              p->nchan, 1, bfx::G4_KT);
+    if (st != BF_XCORR_OK) return st;
+    const int nblk = (p->ninputs + bfx::PR_BLK - 1) / bfx::PR_BLK;
+    TcParams prm;
+    std::memset(&prm, 0, sizeof(prm));
+    prm.out = static_cast<int32_t*>(out);
+    prm.ninputs = p->ninputs;
+    prm.nchan = p->nchan;
+    prm.ntime = p->ntime;
+    prm.tiles_per_chan = nblk * (nblk + 1) / 2;
+    prm.ntiles = static_cast<long long>(prm.tiles_per_chan) * p->nchan;
+    prm.accumulate = accumulate ? 1 : 0;
+    prm.sched = p->d_sched;
+    const long long want = prm.ntiles < p->num_sms ? prm.ntiles : p->num_sms;
+    bfx::xcorr_gauss4_kernel<<<dim3(static_cast<unsigned>(want)), bfx::G4_THREADS, bfx::G4_SMEM_BYTES, stream>>>(tmap, prm);
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(p, e);
+    p->last_launch_count += 1;
+    return BF_XCORR_OK;
+}
+
 // bfXcorrExecuteHost's staging state: released as a whole (also after a partial set-up), pointers nulled
 void release_host_state(bfXcorr plan)
 {
@@ -393,6 +420,7 @@ int bfXcorrExecute(bfXcorr plan, const void* in, void* out, int accumulate, void
     if (cudaGetDevice(&cur) != cudaSuccess || cur != plan->device) return BF_XCORR_INVALID_ARGUMENT;   // the plan's scratch lives on another device
     plan->last_launch_count = 0;
     if (plan->algo == BF_XCORR_ALGO_SIMT) return launch_simt(plan, in, out, accumulate, s);
+    if (plan->algo == BF_XCORR_ALGO_TCGEN05_GAUSS3) return launch_gauss4(plan, in, out, accumulate, s);
     if (plan->d_z) return launch_tcgen05<false>(plan, in, out, accumulate, s);  // S1 fused: dtype handled by the relayout warps
     return plan->dtype == BF_XCORR_CI4 ? launch_tcgen05<true>(plan, in, out, accumulate, s)
                                        : launch_tcgen05<false>(plan, in, out, accumulate, s);
@@ -523,7 +551,15 @@ int bfXcorrGetMaxSafeNtime(bfXcorr plan, unsigned long long* nt)
 int bfXcorrSetAlgo(bfXcorr plan, int algo)
 {
     if (!valid(plan)) return BF_XCORR_INVALID_HANDLE;
-    if (algo != BF_XCORR_ALGO_TCGEN05 && algo != BF_XCORR_ALGO_SIMT) return BF_XCORR_INVALID_ARGUMENT;
+    if (algo != BF_XCORR_ALGO_TCGEN05 && algo != BF_XCORR_ALGO_SIMT && algo != BF_XCORR_ALGO_TCGEN05_GAUSS3) return BF_XCORR_INVALID_ARGUMENT;
+    if (algo == BF_XCORR_ALGO_TCGEN05_GAUSS3) {
+        // the sums re + im fit int8 for 4-bit samples only
+        if (plan->dtype != BF_XCORR_CI4) return BF_XCORR_INVALID_ARGUMENT;
+        const int nblk = (plan->ninputs + bfx::PR_BLK - 1) / bfx::PR_BLK;
+        if (static_cast<unsigned long long>(nblk) * (nblk + 1) / 2 * plan->nchan >= (1ull << 32)) return BF_XCORR_UNSUPPORTED_SHAPE;
+        const cudaError_t e = cudaFuncSetAttribute(bfx::xcorr_gauss4_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bfx::G4_SMEM_BYTES);
+        if (e != cudaSuccess) return cuda_fail(plan, e);
+    }
     plan->algo = algo;
     return BF_XCORR_OK;
 }
@@ -532,6 +568,7 @@ const char* bfXcorrGetKernelName(bfXcorr plan, int accumulate)
 {
     if (!valid(plan)) return "";
     if (plan->algo == BF_XCORR_ALGO_SIMT) return "xcorr_simt_kernel";
+    if (plan->algo == BF_XCORR_ALGO_TCGEN05_GAUSS3) return "xcorr_gauss4_kernel";
     if (!plan->pair) return plan->dtype == BF_XCORR_CI4 ? "xcorr_few_kernel<ci4>" : "xcorr_few_kernel<ci8>";
     if (plan->dtype == BF_XCORR_CI4) return plan->d_z ? "xcorr_pair4_kernel (S1 ring)" : "xcorr_pair4_kernel (in place)";
     if (plan->stripe) {
