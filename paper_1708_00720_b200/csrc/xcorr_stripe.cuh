@@ -263,17 +263,9 @@ xcorr_stripe_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
                     const uint32_t stg_warp = stg_base + wq * TC_STG_BUF_BYTES;
                     int nchunk = (i0 + 15 - j0) / TC_CJ + 1;
                     nchunk = nchunk > 2 ? 2 : nchunk;
-                    if (p.accumulate && lane < 16) {
-                        // the L2 reduce-adds of this tile will want the old visibilities resident
-                        const int i_own = i0 + static_cast<int>(lane);
-                        int n = i_own + 1 - j0;
-                        n = n > PR_BLK ? PR_BLK : n;
-                        if (i_own < p.ninputs && n > 0) {
-                            const long long e0 = static_cast<long long>(i_own) * (i_own + 1) / 2 + j0;
-                            const long long ea = e0 & ~1ll, eb = (e0 + n + 1) & ~1ll;
-                            ptx::bulk_prefetch_l2(out_c + 2 * ea, static_cast<uint32_t>(8 * (eb - ea)));
-                        }
-                    }
+                    // the L2 reduce-adds of this tile will want the old visibilities resident: line prefetches through the
+                    // LSU (a bulk prefetch per row costs a serialised issue loop on the TMA unit: -2.8 %, profiles/round2.md)
+                    if (p.accumulate) tc_prefetch_old(p, lane, out_c, i0, j0, PR_BLK);
                     ptx::mbar_wait(bar_tfull + 8 * buf, bphase);
                     ptx::tc_fence_after();
                     for (int jc = 0; jc < nchunk; ++jc, ++nchunks_done) {
