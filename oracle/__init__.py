@@ -10,6 +10,7 @@ from .xcorr_oracle import (  # noqa: F401
     xcorr,
     xcorr_entries,
     dump,
+    dump_matrix,
     beamform,
     threads,
     set_threads,

@@ -167,6 +167,32 @@ long long xcorr_oracle_dump(int32_t* acc, float* out, long long ncomponents, flo
     return ncomponents;
 }
 
+/* Integration dump with reorder (its optional part; the paper's back end has "efficient data
+ * reordering"): the packed lower triangle becomes the FULL Hermitian matrix in float32,
+ *        out[c][i][j] = ( (float) V.re * scale ,   (float) V.im * scale  )     for j <= i,  V = acc[c][ i(i+1)/2 + j ]
+ *        out[c][i][j] = ( (float) V.re * scale , -((float) V.im * scale) )     for j >  i,  V = acc[c][ j(j+1)/2 + i ]
+ * i.e. the upper triangle is the complex conjugate of the mirrored lower entry (the negation is exact; an imaginary
+ * part of zero becomes -0.0f).  out: [nchan][ninputs][ninputs][2] float32.  The accumulator is cleared afterwards if
+ * zero_acc != 0.  Returns the number of matrix entries written, or -1 on bad arguments. */
+long long xcorr_oracle_dump_matrix(int32_t* acc, float* out, int ninputs, int nchan, float scale, int zero_acc)
+{
+    const long long N = ninputs, C = nchan, B = N * (N + 1) / 2;
+    if (!acc || !out || N <= 0 || C <= 0) return -1;
+    for (long long c = 0; c < C; ++c)
+        for (long long i = 0; i < N; ++i)
+            for (long long j = 0; j < N; ++j) {
+                const long long hi = i >= j ? i : j, lo = i >= j ? j : i;
+                const int32_t* v = acc + 2 * (c * B + hi * (hi + 1) / 2 + lo);
+                const float re = (float)v[0] * scale, im = (float)v[1] * scale;
+                float* o = out + 2 * ((c * N + i) * N + j);
+                o[0] = re;
+                o[1] = j > i ? -im : im;
+            }
+    if (zero_acc)
+        for (long long k = 0; k < 2 * C * B; ++k) acc[k] = 0;
+    return C * N * N;
+}
+
 /* Beamformer on the same span (the GPU stage the paper's deployment runs on the
  * "4+4 complex signed integers"; a "phase-and-sum" of all inputs per beam):
  *

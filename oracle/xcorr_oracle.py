@@ -126,6 +126,21 @@ def dump(acc: np.ndarray, scale: float = 1.0, zero_acc: bool = False) -> np.ndar
     return out
 
 
+def dump_matrix(acc: np.ndarray, ninputs: int, scale: float = 1.0, zero_acc: bool = False) -> np.ndarray:
+    """Integration dump with reorder: int32 [nchan][B][2] -> float32 full Hermitian matrices [nchan][ninputs][ninputs][2]."""
+    nb = ninputs * (ninputs + 1) // 2
+    if acc.dtype != np.int32 or not acc.flags.c_contiguous or acc.ndim != 3 or acc.shape[1:] != (nb, 2):
+        raise ValueError("`acc` must be C-contiguous int32 [nchan][B][2]")
+    nchan = acc.shape[0]
+    out = np.empty((nchan, ninputs, ninputs, 2), dtype=np.float32)
+    fn = _lib().xcorr_oracle_dump_matrix
+    fn.restype = ctypes.c_longlong
+    fn.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_float, ctypes.c_int]
+    if fn(acc.ctypes.data, out.ctypes.data, ninputs, nchan, float(scale), 1 if zero_acc else 0) != nchan * ninputs * ninputs:
+        raise ValueError("xcorr_oracle_dump_matrix rejected its arguments")
+    return out
+
+
 def beamform(x: np.ndarray, w: np.ndarray, ninputs: int, nchan: int, ntime: int, nbeam: int, dtype: int,
              return_nwrap: bool = False):
     """Phase-and-sum beamformer: span x, ci8 weights [nchan][nbeam][ninputs] -> int32 [ntime][nchan][nbeam][2]."""

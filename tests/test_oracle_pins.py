@@ -328,3 +328,40 @@ def test_dump_agrees_with_numpy_float32_arithmetic():
     for scale in (1.0, 1.0 / 1024, 3.0e-5):
         exp = acc.astype(np.float32) * np.float32(scale)
         np.testing.assert_array_equal(oracle.dump(acc, scale), exp)
+
+
+# ---- integration dump with reorder (optional part): packed triangle -> full Hermitian float32 matrix ----
+def test_dump_matrix_worked_example_and_hermitian():
+    """The hand-worked N = 3 visibilities of tests/golden/worked_example_n3.txt as a full matrix, written out by hand:
+    row i, column j holds V_ij below / on the diagonal and conj(V_ji) above it."""
+    g = read_golden("worked_example_n3.txt")
+    acc = np.array([[(r, m) for _, r, m in g["v"]]], dtype=np.int32)       # [1][6][2]: (17,0) (-9,22) (46,0) (1,0) (-15,3) (34,0)
+    m = oracle.dump_matrix(acc, 3, 1.0)
+    z = m[0, ..., 0] + 1j * m[0, ..., 1]
+    exp = np.array([[17, -9 - 22j, 1 - 0j], [-9 + 22j, 46, -15 - 3j], [1 + 0j, -15 + 3j, 34]])
+    assert np.array_equal(z, exp)
+    assert np.array_equal(z, z.conj().T)                                    # Hermitian
+    assert np.signbit(m[0, 0, 2, 1]) and not np.signbit(m[0, 2, 0, 1])      # conj of a zero imaginary part is -0.0
+    half = oracle.dump_matrix(acc, 3, 0.5)
+    assert np.array_equal(half, m * np.float32(0.5))
+
+
+def test_dump_matrix_agrees_with_dump_and_numpy_indexing():
+    """Independent construction: oracle.dump's floats scattered into a matrix with numpy's tril indices; zeroing."""
+    rng = np.random.default_rng(21)
+    N, C = 11, 3
+    nb = N * (N + 1) // 2
+    acc = rng.integers(-2**31, 2**31, size=(C, nb, 2), dtype=np.int64).astype(np.int32)
+    scale = 0.37
+    flat = oracle.dump(acc.copy(), scale)
+    exp = np.zeros((C, N, N, 2), dtype=np.float32)
+    ii, jj = np.tril_indices(N)                                             # row-major lower triangle = the packed order
+    exp[:, ii, jj] = flat
+    exp[:, jj, ii, 0] = flat[..., 0]
+    off = ii != jj
+    exp[:, jj[off], ii[off], 1] = -flat[:, off, 1]
+    work = acc.copy()
+    got = oracle.dump_matrix(work, N, scale, zero_acc=True)
+    assert np.array_equal(got.view(np.uint32)[:, ii, jj], exp.view(np.uint32)[:, ii, jj])
+    assert np.array_equal(got, exp) and not work.any()
+    assert np.array_equal(oracle.dump_matrix(acc.copy(), N, scale), got)    # zero_acc does not change the output
