@@ -152,6 +152,16 @@ int bfXcorrExecuteHost(bfXcorr plan, const void* in_host, void* out_dev, void* o
  *   errors : INVALID_HANDLE; INVALID_POINTER (NULL or misaligned); DEVICE_ERROR. */
 int bfXcorrDump(bfXcorr plan, void* acc, void* out, float scale, int zero_acc, void* stream);
 
+/* Integration dump with reorder (the paper's back end has "efficient data reordering"): as
+ * bfXcorrDump, but the packed lower triangle is written out as the FULL Hermitian matrix
+ *   out[c][i][j] = (float) V[c][i][j] * scale             for j <= i
+ *   out[c][i][j] = conj( out[c][j][i] )                   for j >  i   (exact; a zero imaginary part becomes -0.0f)
+ *   acc    : as bfXcorrDump.
+ *   out    : DEVICE pointer, [nchan][ninputs][ninputs][2] float32 = nchan * ninputs^2 * 8 bytes, 8-byte aligned, must not
+ *            overlap `acc`.
+ *   errors : as bfXcorrDump. */
+int bfXcorrDumpMatrix(bfXcorr plan, void* acc, void* out, float scale, int zero_acc, void* stream);
+
 /* Measurement aid (the same-mix HBM ceiling): a no-math streaming kernel that moves exactly
  * the path's algorithmic bytes with coalesced, contiguous accesses -- reads the span once, and writes the visibility
  * buffer once (accumulate = 0) or reads, increments and rewrites it (accumulate != 0).  It computes nothing of the

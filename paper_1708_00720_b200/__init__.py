@@ -22,6 +22,7 @@ from .binding import (  # noqa: F401
     bfXcorrCreate,
     bfXcorrDestroy,
     bfXcorrDump,
+    bfXcorrDumpMatrix,
     bfXcorrExecute,
     bfXcorrExecuteHost,
     bfXcorrGetInputBytes,

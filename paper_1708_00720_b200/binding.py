@@ -37,6 +37,7 @@ SIGNATURES = {
     "bfXcorrGetLastCudaError": (_i, [_vp, _ip]),
     "bfXcorrExecuteHost": (_i, [_vp, _vp, _vp, _vp, _i, _vp]),
     "bfXcorrDump": (_i, [_vp, _vp, _vp, ctypes.c_float, _i, _vp]),
+    "bfXcorrDumpMatrix": (_i, [_vp, _vp, _vp, ctypes.c_float, _i, _vp]),
     "bfXcorrMemoryProbe": (_i, [_vp, _vp, _vp, _i, _vp]),
     "bfXcorrGetStatusString": (ctypes.c_char_p, [_i]),
     "bfXcorrGetKernelName": (ctypes.c_char_p, [_vp, _i]),
@@ -104,6 +105,12 @@ def bfXcorrDump(plan: _vp, acc_ptr: int, out_ptr: int, scale: float = 1.0, zero_
     """acc_ptr: device int32 visibilities; out_ptr: device float32 buffer of the same size."""
     _check(lib().bfXcorrDump(plan, _vp(acc_ptr), _vp(out_ptr), ctypes.c_float(scale), 1 if zero_acc else 0, _vp(stream)),
            "bfXcorrDump")
+
+
+def bfXcorrDumpMatrix(plan: _vp, acc_ptr: int, out_ptr: int, scale: float = 1.0, zero_acc: bool = False, stream: int = 0) -> None:
+    """acc_ptr: device int32 visibilities; out_ptr: device float32 [nchan][ninputs][ninputs][2] (full Hermitian matrices)."""
+    _check(lib().bfXcorrDumpMatrix(plan, _vp(acc_ptr), _vp(out_ptr), ctypes.c_float(scale), 1 if zero_acc else 0, _vp(stream)),
+           "bfXcorrDumpMatrix")
 
 
 def bfXcorrMemoryProbe(plan: _vp, in_ptr: int, out_ptr: int, accumulate: bool, stream: int = 0) -> None:

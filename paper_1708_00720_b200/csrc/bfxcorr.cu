@@ -493,6 +493,26 @@ int bfXcorrDump(bfXcorr plan, void* acc, void* out, float scale, int zero_acc, v
     return BF_XCORR_OK;
 }
 
+int bfXcorrDumpMatrix(bfXcorr plan, void* acc, void* out, float scale, int zero_acc, void* stream)
+{
+    if (!valid(plan)) return BF_XCORR_INVALID_HANDLE;
+    if (!acc || !out) return BF_XCORR_INVALID_POINTER;
+    if ((reinterpret_cast<uintptr_t>(acc) & 15u) || (reinterpret_cast<uintptr_t>(out) & 7u)) return BF_XCORR_INVALID_POINTER;
+    const int nb = (plan->ninputs + bfx::DM_TILE - 1) / bfx::DM_TILE;
+    const long long tiles = static_cast<long long>(nb) * (nb + 1) / 2;
+    long long ychan = plan->nchan;
+    const long long cap = (64ll * plan->num_sms + tiles - 1) / tiles;   // enough CTAs to fill the machine, channels strided beyond that
+    if (ychan > cap) ychan = cap;
+    if (ychan > 65535) ychan = 65535;
+    plan->last_launch_count = 0;
+    bfx::xcorr_dump_matrix_kernel<<<dim3(static_cast<unsigned>(tiles), static_cast<unsigned>(ychan)), 256, 0, static_cast<cudaStream_t>(stream)>>>(
+        static_cast<int32_t*>(acc), static_cast<float2*>(out), plan->ninputs, plan->nchan, scale, zero_acc ? 1 : 0);
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(plan, e);
+    plan->last_launch_count = 1;
+    return BF_XCORR_OK;
+}
+
 int bfXcorrMemoryProbe(bfXcorr plan, const void* in, void* out, int accumulate, void* stream)
 {
     if (!valid(plan)) return BF_XCORR_INVALID_HANDLE;
