@@ -68,7 +68,8 @@ typedef enum bfXcorrStatus_ {
     BF_XCORR_UNSUPPORTED_SHAPE = 5,  /* see bfXcorrCreate                                       */
     BF_XCORR_UNSUPPORTED_DEVICE = 6, /* no CUDA device of compute capability 10.x               */
     BF_XCORR_MEM_ALLOC_FAILED = 7,
-    BF_XCORR_DEVICE_ERROR = 8        /* a CUDA call failed; see bfXcorrGetLastCudaError         */
+    BF_XCORR_DEVICE_ERROR = 8,       /* a CUDA call failed; see bfXcorrGetLastCudaError         */
+    BF_XCORR_SCRATCH_LIMIT = 9       /* bfXcorrExecuteNoAlloc: the span needs more scratch than the fixed buffer holds */
 } bfXcorrStatus;
 
 /* Which kernel bfXcorrExecute launches.  TCGEN05 is the product path and the default: unpack-and-transpose
@@ -169,6 +170,35 @@ int bfXcorrDumpMatrix(bfXcorr plan, void* acc, void* out, float scale, int zero_
  * bandwidth it reaches as roofline.same_mix_peak.
  *   in, out, stream : as bfXcorrExecute (sizes from the plan).  errors: as bfXcorrExecute. */
 int bfXcorrMemoryProbe(bfXcorr plan, const void* in, void* out, int accumulate, void* stream);
+
+/* One span, with NO device-memory allocation anywhere: for callers that cannot call cudaMalloc (a tight serving loop,
+ * a harness that forbids it).  No plan: the geometry is passed with every call.  The same tensor-core kernels as
+ * bfXcorrExecute with the default algorithm, chosen by the same rule, and the same result bit for bit
+ * (out[c][i(i+1)/2 + j] = (accumulate ? out : 0) + sum_t x_i conj(x_j), PAPER.md:378 / SURVEY.md 8c); what differs is
+ * where their scratch lives.  A plan allocates it at bfXcorrCreate (the tile scheduler's counters, and for spans that
+ * take the unpack-and-transpose stage through the L2-resident S1 ring -- ci8 spans of more than 1024 samples, and spans
+ * of more than 1024 inputs whose consecutive samples of a channel lie more than 1 MiB apart -- the ring of channel slabs
+ * and two progress counters per channel).  Here all of it is one file-scope `static __device__` array of BF_XCORR_NOALLOC_SCRATCH_BYTES that every GPU
+ * holds from the moment it loads the library until the process exits.
+ *   in, out, accumulate, stream : as bfXcorrExecute (DEVICE pointers, 16-byte aligned; the caller owns them).
+ *   ninputs, nchan, ntime, dtype : as bfXcorrCreate, same limits.
+ * Limits of the fixed scratch (BF_XCORR_SCRATCH_LIMIT, nothing launched): a span that needs the S1 ring must have at
+ * most BF_XCORR_NOALLOC_MAX_RING_CHANNELS channels and the smallest workable ring (the channels in flight, twice, plus 4
+ * slabs of ntime * ninputs * 2 bytes, ci4: ntime * ninputs) must fit BF_XCORR_NOALLOC_RING_BYTES; BASELINE.json's five configs all fit (only
+ * configs[3] uses the ring: 14 slabs of 4 MiB).  Spans read in place need 32 bytes and are never rejected.
+ * The array is shared by every call on the device and keeps the last call's contents: each call first clears, on
+ * `stream`, the counters it needs at zero.  Two calls whose work overlaps on the GPU (different streams, or different
+ * host threads) therefore race -- order them on one stream or with events; bfXcorrExecute on a plan is not affected.
+ * The first call on a device also does that device's one-time set-up (the array's address, kernel attributes, the
+ * tensor-map encoder): no allocation either, but make it outside a stream capture.  Never calls cudaMalloc, cudaFree or
+ * an allocating library routine.
+ *   errors : as bfXcorrCreate and bfXcorrExecute for the arguments; BF_XCORR_UNSUPPORTED_DEVICE without a compute
+ *            capability 10.x device; BF_XCORR_SCRATCH_LIMIT as above; BF_XCORR_DEVICE_ERROR if a CUDA call fails. */
+#define BF_XCORR_NOALLOC_RING_BYTES (64ull << 20)
+#define BF_XCORR_NOALLOC_MAX_RING_CHANNELS 65536
+#define BF_XCORR_NOALLOC_SCRATCH_BYTES (1024ull + 16ull * BF_XCORR_NOALLOC_MAX_RING_CHANNELS + BF_XCORR_NOALLOC_RING_BYTES)
+int bfXcorrExecuteNoAlloc(const void* in, void* out, int ninputs, int nchan, int ntime, int dtype, int accumulate,
+                          void* stream);
 
 /* Static string for a status code (never NULL). */
 const char* bfXcorrGetStatusString(int status);

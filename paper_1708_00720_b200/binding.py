@@ -15,6 +15,7 @@ from . import _build
 BF_XCORR_CI4 = 4
 BF_XCORR_CI8 = 8
 BF_XCORR_OK = 0
+BF_XCORR_SCRATCH_LIMIT = 9
 BF_XCORR_ALGO_TCGEN05 = 0
 BF_XCORR_ALGO_SIMT = 1
 BF_XCORR_ALGO_TCGEN05_GAUSS3 = 2
@@ -39,6 +40,7 @@ SIGNATURES = {
     "bfXcorrDump": (_i, [_vp, _vp, _vp, ctypes.c_float, _i, _vp]),
     "bfXcorrDumpMatrix": (_i, [_vp, _vp, _vp, ctypes.c_float, _i, _vp]),
     "bfXcorrMemoryProbe": (_i, [_vp, _vp, _vp, _i, _vp]),
+    "bfXcorrExecuteNoAlloc": (_i, [_vp, _vp, _i, _i, _i, _i, _i, _vp]),
     "bfXcorrGetStatusString": (ctypes.c_char_p, [_i]),
     "bfXcorrGetKernelName": (ctypes.c_char_p, [_vp, _i]),
     # include/bfbeamform.h
@@ -116,6 +118,13 @@ def bfXcorrDumpMatrix(plan: _vp, acc_ptr: int, out_ptr: int, scale: float = 1.0,
 def bfXcorrMemoryProbe(plan: _vp, in_ptr: int, out_ptr: int, accumulate: bool, stream: int = 0) -> None:
     """No-math streaming kernel with the path's HBM access mix (measurement aid); `out` is left with meaningless values."""
     _check(lib().bfXcorrMemoryProbe(plan, _vp(in_ptr), _vp(out_ptr), 1 if accumulate else 0, _vp(stream)), "bfXcorrMemoryProbe")
+
+
+def bfXcorrExecuteNoAlloc(in_ptr: int, out_ptr: int, ninputs: int, nchan: int, ntime: int, dtype: int, accumulate: bool,
+                          stream: int = 0) -> None:
+    """One span without a plan and without any device allocation (scratch in the library's static device array)."""
+    _check(lib().bfXcorrExecuteNoAlloc(_vp(in_ptr), _vp(out_ptr), ninputs, nchan, ntime, dtype, 1 if accumulate else 0, _vp(stream)),
+           "bfXcorrExecuteNoAlloc")
 
 
 def bfXcorrDestroy(plan: _vp) -> None:

@@ -3,6 +3,7 @@
 #include <cstdint>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 
 #include <cuda.h>
@@ -295,6 +296,76 @@ int launch_simt(bfXcorr p, const void* in, void* out, int accumulate, cudaStream
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(p, e);
     p->last_launch_count += 1;
+    return BF_XCORR_OK;
+}
+
+// ---- bfXcorrExecuteNoAlloc: every kernel's scratch in one static device array (include/bfxcorr.h) ----------------
+// layout: [0, 1024) scheduler words | [1024, 1024 + 16 * MAX_RING_CHANNELS) ready[nchan], done[nchan] | S1 ring
+constexpr size_t kNaFlagsOff = 1024;
+constexpr size_t kNaRingOff = kNaFlagsOff + 16ull * BF_XCORR_NOALLOC_MAX_RING_CHANNELS;
+static_assert(kNaRingOff % 1024 == 0, "ring slabs are TMA sources");
+static_assert(kNaRingOff + BF_XCORR_NOALLOC_RING_BYTES == BF_XCORR_NOALLOC_SCRATCH_BYTES, "header and layout agree");
+
+// In host code this name is a host-side stand-in, not a device address: na_device_state() asks the runtime for the
+// address on the current device (cudaGetSymbolAddress) and the kernels get that pointer.
+static __device__ __align__(256) unsigned char g_noalloc_scratch[BF_XCORR_NOALLOC_SCRATCH_BYTES];
+
+struct NaDevice {
+    bool ready;
+    unsigned char* scratch;   // device address of g_noalloc_scratch on this device
+    int num_sms;
+};
+constexpr int kNaMaxDevices = 64;
+NaDevice g_na_device[kNaMaxDevices];   // zero-initialised
+EncodeTiledFn g_na_encode = nullptr;
+std::mutex g_na_mutex;
+
+// One-time set-up of the current device `dev` (no allocation).  Returns a status; *out valid on BF_XCORR_OK.
+int na_device_state(int dev, NaDevice* out)
+{
+    if (dev < 0 || dev >= kNaMaxDevices) return BF_XCORR_UNSUPPORTED_DEVICE;
+    std::lock_guard<std::mutex> lock(g_na_mutex);
+    NaDevice& d = g_na_device[dev];
+    if (!d.ready) {
+        int major = 0, sms = 0;
+        if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess || major != 10) {
+            cudaGetLastError();
+            return BF_XCORR_UNSUPPORTED_DEVICE;
+        }
+        if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0) return BF_XCORR_UNSUPPORTED_DEVICE;
+        if (!g_na_encode) {
+            void* fn = nullptr;
+            cudaDriverEntryPointQueryResult qres;
+            const cudaError_t eq = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+            if (eq != cudaSuccess || qres != cudaDriverEntryPointSuccess || !fn) return BF_XCORR_UNSUPPORTED_DEVICE;
+            g_na_encode = reinterpret_cast<EncodeTiledFn>(fn);
+        }
+        void* ptr = nullptr;
+        cudaError_t e = cudaGetSymbolAddress(&ptr, g_noalloc_scratch);
+        if (e == cudaSuccess && !ptr) e = cudaErrorInvalidSymbol;
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(bfx::xcorr_few_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bfx::FwCfg<true>::kSmemBytes);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(bfx::xcorr_few_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bfx::FwCfg<false>::kSmemBytes);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(bfx::xcorr_pair4_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bfx::P4_SMEM_BYTES);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(bfx::xcorr_pair_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bfx::PR_SMEM_BYTES);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(bfx::xcorr_stripe_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bfx::StCfg<true, false>::kSmemBytes);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(bfx::xcorr_stripe_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bfx::StCfg<false, true>::kSmemBytes);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(bfx::xcorr_stripe_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bfx::StCfg<false, false>::kSmemBytes);
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            return BF_XCORR_DEVICE_ERROR;
+        }
+        d.scratch = static_cast<unsigned char*>(ptr);
+        d.num_sms = sms;
+        d.ready = true;
+    }
+    *out = d;
     return BF_XCORR_OK;
 }
 
@@ -614,6 +685,78 @@ int bfXcorrGetLastCudaError(bfXcorr plan, int* cuda_error)
     return BF_XCORR_OK;
 }
 
+int bfXcorrExecuteNoAlloc(const void* in, void* out, int ninputs, int nchan, int ntime, int dtype, int accumulate, void* stream)
+{
+    // arguments: bfXcorrCreate's and bfXcorrExecute's checks, in their order
+    if (ninputs <= 0 || nchan <= 0 || ntime <= 0 || ntime > 65535) return BF_XCORR_INVALID_ARGUMENT;
+    if (dtype != BF_XCORR_CI4 && dtype != BF_XCORR_CI8) return BF_XCORR_INVALID_DTYPE;
+    if ((static_cast<unsigned long long>(ninputs) * bytes_per_sample(dtype)) % 16ull != 0) return BF_XCORR_UNSUPPORTED_SHAPE;
+    if (ninputs > 32768) return BF_XCORR_UNSUPPORTED_SHAPE;
+    if (!in || !out) return BF_XCORR_INVALID_POINTER;
+    if ((reinterpret_cast<uintptr_t>(in) & 15u) || (reinterpret_cast<uintptr_t>(out) & 15u)) return BF_XCORR_INVALID_POINTER;
+    int ndev = 0, dev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev <= 0 || cudaGetDevice(&dev) != cudaSuccess) {
+        cudaGetLastError();
+        return BF_XCORR_UNSUPPORTED_DEVICE;
+    }
+    NaDevice nd;
+    const int st = na_device_state(dev, &nd);
+    if (st != BF_XCORR_OK) return st;
+
+    // A plan on the stack, filled as bfXcorrCreate fills one (same kernel choice, same tile counts), whose scratch
+    // pointers lead into the static array; it lives for this call only.
+    bfXcorr_impl plan;
+    std::memset(&plan, 0, sizeof(plan));
+    plan.magic = kMagic;
+    plan.ninputs = ninputs;
+    plan.nchan = nchan;
+    plan.ntime = ntime;
+    plan.dtype = dtype;
+    plan.algo = BF_XCORR_ALGO_TCGEN05;
+    plan.device = dev;
+    plan.num_sms = nd.num_sms;
+    plan.encode = g_na_encode;
+    const bool pair = ninputs > 64;
+    const int nblk = (ninputs + bfx::PR_BLK - 1) / bfx::PR_BLK;
+    plan.pair = pair;
+    plan.stripe = BFX_STRIPE && pair && dtype == BF_XCORR_CI8 && ntime <= bfx::ST_MAXKB * bfx::TC_KT;
+    plan.tiles_per_chan = pair ? nblk * (nblk + 1) / 2 : 1;
+    if (pair && static_cast<unsigned long long>(plan.tiles_per_chan) * nchan >= (1ull << 32)) return BF_XCORR_UNSUPPORTED_SHAPE;
+    plan.d_sched = reinterpret_cast<unsigned long long*>(nd.scratch);
+    size_t clear_bytes = 4 * sizeof(unsigned long long);   // the scheduler words
+    const bool near = static_cast<unsigned long long>(nchan) * ninputs * bytes_per_sample(dtype) <= (static_cast<unsigned long long>(BFX_DIRECT_STRIDE_KB) << 10);
+    const bool direct = pair && (plan.stripe || dtype == BF_XCORR_CI4) &&
+                        (nblk <= BFX_DIRECT_MAX_BLK || near || (dtype == BF_XCORR_CI4 && !BFX_P4_RING));
+    if (pair && !direct) {
+        // the S1 ring: bfXcorrCreate's sizing (channels in flight, doubled, + 2 + look-ahead), the look-ahead cut down
+        // to what the fixed buffer holds but never below the 2 slabs bfXcorrCreate itself would accept
+        if (nchan > BF_XCORR_NOALLOC_MAX_RING_CHANNELS) return BF_XCORR_SCRATCH_LIMIT;
+        const unsigned long long slab = static_cast<unsigned long long>(ntime) * ring_row_bytes(&plan);
+        const int per_chan = plan.stripe ? nblk : plan.tiles_per_chan;
+        const int window = (plan.num_sms / 2 + per_chan - 1) / per_chan;
+        long long ahead = static_cast<long long>(((plan.stripe ? static_cast<unsigned long long>(BFX_ST_AHEAD_MB) : 16ull) << 20) / slab);
+        if (ahead < 2) ahead = 2;
+        long long ring = 2 * window + 2 + ahead;
+        long long ring_min = 2 * window + 2 + 2;
+        if (ring > nchan) ring = nchan;
+        if (ring_min > nchan) ring_min = nchan;
+        const long long fits = static_cast<long long>(BF_XCORR_NOALLOC_RING_BYTES / slab);
+        if (fits < ring_min) return BF_XCORR_SCRATCH_LIMIT;
+        if (ring > fits) ring = fits;
+        plan.ring_w = static_cast<int>(ring);
+        plan.d_z = nd.scratch + kNaRingOff;
+        plan.d_flags = reinterpret_cast<unsigned long long*>(nd.scratch + kNaFlagsOff);
+        clear_bytes = kNaFlagsOff + 2ull * nchan * sizeof(unsigned long long);   // ... and ready[] / done[], which count from zero
+    }
+    // the array keeps what the last call (of any shape) left in it
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    const cudaError_t e = cudaMemsetAsync(nd.scratch, 0, clear_bytes, s);
+    if (e != cudaSuccess) return cuda_fail(nullptr, e);
+    if (plan.d_z) return launch_tcgen05<false>(&plan, in, out, accumulate, s);
+    return dtype == BF_XCORR_CI4 ? launch_tcgen05<true>(&plan, in, out, accumulate, s)
+                                 : launch_tcgen05<false>(&plan, in, out, accumulate, s);
+}
+
 const char* bfXcorrGetStatusString(int status)
 {
     switch (status) {
@@ -626,6 +769,7 @@ const char* bfXcorrGetStatusString(int status)
         case BF_XCORR_UNSUPPORTED_DEVICE: return "BF_XCORR_UNSUPPORTED_DEVICE";
         case BF_XCORR_MEM_ALLOC_FAILED: return "BF_XCORR_MEM_ALLOC_FAILED";
         case BF_XCORR_DEVICE_ERROR: return "BF_XCORR_DEVICE_ERROR";
+        case BF_XCORR_SCRATCH_LIMIT: return "BF_XCORR_SCRATCH_LIMIT";
         default: return "BF_XCORR_UNKNOWN_STATUS";
     }
 }
