@@ -227,7 +227,13 @@ xcorr_pair4_kernel(const __grid_constant__ CUtensorMap tmap, const TcParams p)
                     ptx::mbar_wait(bar_full + 8 * stage, phase);
                     // the stage lives in this CTA's shared memory and is complete (observed through the local barrier):
                     // a plain remote arrival is enough, a cluster-scope release would cost a MEMBAR per stage
+                    // (BFX_RING_ARRIVE >= 1, xcorr_pair.cuh: the build that follows the PTX memory model to the letter --
+                    // tests/test_gpu_conformant_build.py runs it against this one)
+#if BFX_RING_ARRIVE >= 1
+                    if (lane == 0) ptx::mbar_arrive_release_cluster_addr(lead_full + 8 * stage);
+#else
                     if (lane == 0) ptx::mbar_arrive_cluster_addr(lead_full + 8 * stage);
+#endif
                     __syncwarp();
                     if (++stage == S) { stage = 0; phase ^= 1; }
                 }
