@@ -201,6 +201,22 @@ def spaced_channels(nchan: int, n: int):
     return sorted(set(int(round(k * (nchan - 1) / max(1, n - 1))) for k in range(n))) if n > 1 else [0]
 
 
+# the oracle legs' input: at most this many bytes of span per sampled slab (the seeded generator works in int64 temporaries,
+# a dozen bytes per sample while it runs; cfg5 has 16384 cheap channels and the sample would otherwise grow to the whole span)
+ORACLE_SAMPLE_MAX_BYTES = 1 << 30
+
+
+def channel_slab_numpy(cfg, span: int, chans):
+    """generate_channel_slab in channel chunks of <= 32 Mi samples (on the GPU when there is one), as one numpy array."""
+    import numpy as np
+    import torch
+    from xcorr_inputs import generate_channel_slab
+    dev = "cuda" if torch.cuda.is_available() else "cpu"
+    per = max(1, (32 << 20) // (cfg.ntime * cfg.ninputs))
+    parts = [generate_channel_slab(cfg, span, chans[a:a + per], device=dev).cpu().numpy() for a in range(0, len(chans), per)]
+    return parts[0] if len(parts) == 1 else np.concatenate(parts, axis=1)
+
+
 def oracle_sample(cfg, target_s: float):
     """Time the oracle (as it stands) on a bounded channel subset of the workload, all spans accumulated.
     Returns (seconds, channels, threads, oracle result [len(channels)][B][2], one-thread info)."""
@@ -209,14 +225,15 @@ def oracle_sample(cfg, target_s: float):
     nthreads = oracle.threads()
     # calibration: one channel per thread, one span
     chans = spaced_channels(cfg.nchan, min(cfg.nchan, nthreads))
-    x = generate_channel_slab(cfg, 0, chans).numpy()
+    x = channel_slab_numpy(cfg, 0, chans)
     t0 = time.perf_counter()
     oracle.xcorr(x, cfg.ninputs, len(chans), cfg.ntime, cfg.dtype)
     tcal = time.perf_counter() - t0
     per_wave = tcal / len(chans) * min(len(chans), nthreads)  # seconds of one "wave" of nthreads channels, one span
     waves = max(1, int(target_s / max(per_wave * cfg.nspans, 1e-9)))
-    chans = spaced_channels(cfg.nchan, min(cfg.nchan, waves * nthreads))
-    slabs = [generate_channel_slab(cfg, s, chans).numpy() for s in range(cfg.nspans)]
+    cap = max(nthreads, ORACLE_SAMPLE_MAX_BYTES // (cfg.ntime * cfg.ninputs * cfg.bytes_per_sample))
+    chans = spaced_channels(cfg.nchan, min(cfg.nchan, waves * nthreads, cap))
+    slabs = [channel_slab_numpy(cfg, s, chans) for s in range(cfg.nspans)]
     t0 = time.perf_counter()
     out = oracle.xcorr(slabs[0], cfg.ninputs, len(chans), cfg.ntime, cfg.dtype)
     for s in range(1, cfg.nspans):
@@ -340,9 +357,10 @@ def run_beamform(args, cfg):
     if not args.no_cpu_baseline:
         nthreads = oracle.threads()
         per_chan_macs = float(T) * K * N
-        nch = int(max(1, min(C, args.cpu_seconds * 2.0e8 * nthreads / per_chan_macs)))   # ~2e8 complex MAC/s/thread
+        nch = int(max(1, min(C, args.cpu_seconds * 2.0e8 * nthreads / per_chan_macs,   # ~2e8 complex MAC/s/thread
+                             max(nthreads, ORACLE_SAMPLE_MAX_BYTES // (T * N * cfg.bytes_per_sample)))))
         chans = sorted(set(int(round(k * (C - 1) / max(1, nch - 1))) for k in range(nch))) if nch > 1 else [0]
-        xs = generate_channel_slab(cfg, 0, chans).numpy()
+        xs = channel_slab_numpy(cfg, 0, chans)
         ws = generate_weights(cfg.seed, C, K, N, channels=chans).numpy()
         t0 = time.perf_counter()
         oracle.beamform(xs, ws, N, len(chans), T, K, cfg.dtype)
