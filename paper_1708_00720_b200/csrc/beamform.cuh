@@ -21,7 +21,10 @@
 // in the L2 while its sample blocks go by.
 //
 // Roles (512 threads, one CTA per SM): warp 0 span producer (TMA boxes of 128 span bytes x 128 samples of one channel:
-// ci8 lands 128B-swizzled straight in the operand stage, ci4 lands raw in a ring), warp 3 weight producer (ci4 only; for
+// ci8 lands 128B-swizzled straight in the operand stage -- two adjacent 128-byte pieces per box through a 5-d view of
+// the span where the shape allows it (rows a multiple of 256 bytes, samples a multiple of 8, three stages fit), which
+// the memory system serves much faster when a channel's samples lie pages apart: 76 -> 92 % of the HBM copy peak on
+// BASELINE.json configs[2], 70 -> 102 % on configs[3] (profiles/round2.md) --, ci4 lands raw in a ring), warp 3 weight producer (ci4 only; for
 // ci8 warp 0 loads both), warp 1 MMA issuer, warp 2 TMEM allocator, warps 4..7 epilogue (TMEM -> registers -> shared
 // staging -> global, eight lanes per 128-byte row piece), warps 8..15 (ci4 only) widen raw rows into the 128B-swizzled K-major int8 layout the
 // UMMA descriptor expects.  TMA keeps every free stage in flight (up to 128 KB per SM), which register-staged loads
@@ -54,6 +57,7 @@ struct BmParams {
     int group;       // adjacent channels per scheduling group
     int stages;      // operand stages
     int raw_stages;  // raw ci4 stages (0 for ci8)
+    int pw;          // ci8: 128-byte row pieces per K stage and span box (1, or 2 with the 5-d span map: see the producer)
     long long nunits;
 };
 
@@ -72,13 +76,13 @@ __device__ __forceinline__ BmUnit bm_decode(const BmParams& p, long long u)
     return BmUnit{cg * p.group + (r - tb * gl), tb * BM_MT};
 }
 
-// UMMA shared-memory descriptor, K-major, SWIZZLE_128B: rows of 128 bytes, 8-row atoms 1024 bytes apart
-__device__ __forceinline__ uint64_t bm_smem_desc(uint32_t saddr)
+// UMMA shared-memory descriptor, K-major, SWIZZLE_128B: rows of 128 bytes, 8-row atoms `sbo` bytes apart (1024: a dense tile)
+__device__ __forceinline__ uint64_t bm_smem_desc(uint32_t saddr, uint32_t sbo = 1024u)
 {
     uint64_t d = 0;
     d |= static_cast<uint64_t>((saddr >> 4) & 0x3FFF);
     d |= static_cast<uint64_t>(1) << 16;
-    d |= static_cast<uint64_t>((1024u >> 4) & 0x3FFF) << 32;
+    d |= static_cast<uint64_t>((sbo >> 4) & 0x3FFF) << 32;
     d |= static_cast<uint64_t>(1) << 46;
     d |= static_cast<uint64_t>(2) << 61;
     return d;
@@ -100,7 +104,8 @@ beamform_kernel(const __grid_constant__ CUtensorMap xmap, const __grid_constant_
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
     const uint32_t w_tile = static_cast<uint32_t>(p.nb2) * 128u;
-    const uint32_t stage_bytes = KH * (A_TILE + w_tile);
+    const int kh = CI4 ? KH : p.pw;             // 128-byte K tiles per stage
+    const uint32_t stage_bytes = kh * (A_TILE + w_tile);
     const int S = p.stages;
     const int R = p.raw_stages;
     const uint32_t raw_base = smem_base + S * stage_bytes;      // [R] raw ci4 tiles [128 samples][128 bytes]
@@ -165,9 +170,19 @@ beamform_kernel(const __grid_constant__ CUtensorMap xmap, const __grid_constant_
                     ptx::mbar_wait(bar_empty + 8 * stage, phase ^ 1);
                     if (lane == 0) {
                         const uint32_t dst = smem_base + stage * stage_bytes;
-                        ptx::mbar_expect_tx(bar_full + 8 * stage, A_TILE + w_tile);
-                        ptx::tma_load_3d_hint(dst, &xmap, bar_full + 8 * stage, ks * 128, un.c, un.t0, pol_first);
-                        ptx::tma_load_2d_hint(dst + A_TILE, &wmap, bar_full + 8 * stage, ks * KS, un.c * p.nb2, pol_last);
+                        ptx::mbar_expect_tx(bar_full + 8 * stage, kh * (A_TILE + w_tile));
+                        if (p.pw == 1) {
+                            ptx::tma_load_3d_hint(dst, &xmap, bar_full + 8 * stage, ks * 128, un.c, un.t0, pol_first);
+                        } else {
+                            // 5-d view of the span {128 B, 8 samples, row pieces, channels, 8-sample groups}, box {128, 8, pw, 1, 16}:
+                            // the requests of one 8-sample group walk the SAME eight pages once per piece, which the memory
+                            // system serves faster than a new page per request (profiles/round2.md: 650 against 842 cycles per
+                            // 16 KiB with every SM loading).  In shared memory piece h is the canonical K-major tile with its
+                            // 8-row atoms pw KiB apart.
+                            ptx::tma_load_5d_hint(dst, &xmap, bar_full + 8 * stage, 0, 0, ks * p.pw, un.c, un.t0 >> 3, pol_first);
+                        }
+                        for (int h = 0; h < kh; ++h)
+                            ptx::tma_load_2d_hint(dst + kh * A_TILE + h * w_tile, &wmap, bar_full + 8 * stage, (ks * kh + h) * 128, un.c * p.nb2, pol_last);
                     }
                 }
                 __syncwarp();
@@ -208,10 +223,10 @@ beamform_kernel(const __grid_constant__ CUtensorMap xmap, const __grid_constant_
                 ptx::tc_fence_after();
                 if (lane == 0) {
                     const uint32_t abase = smem_base + stage * stage_bytes;
-                    const uint32_t wbase = abase + KH * A_TILE;
-#pragma unroll
-                    for (int h = 0; h < KH; ++h) {
-                        const uint64_t adesc = bm_smem_desc(abase + h * A_TILE);
+                    const uint32_t wbase = abase + kh * A_TILE;
+                    for (int h = 0; h < kh; ++h) {
+                        // ci4: dense tiles one after the other; ci8: piece h of the span box (atoms kh KiB apart; kh = 1: dense)
+                        const uint64_t adesc = CI4 ? bm_smem_desc(abase + h * A_TILE) : bm_smem_desc(abase + h * 1024u, kh * 1024u);
                         const uint64_t bdesc = bm_smem_desc(wbase + h * w_tile);
 #pragma unroll
                         for (int k = 0; k < 4; ++k)

@@ -16,6 +16,10 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
+// ci8: row pieces per span box (2: the 5-d span map of beamform.cuh, where the shape allows it; 1: always the 3-d map)
+#ifndef BFX_BM_PW
+#define BFX_BM_PW 2
+#endif
 #ifndef BFX_BM_GROUP_MB
 #define BFX_BM_GROUP_MB 8
 #endif
@@ -116,11 +120,20 @@ int bfBeamformCreate(bfBeamform* plan, int ninputs, int nchan, int ntime, int nb
     q.row_in = row_in;
     q.nb2 = (2 * nbeam + 2 + 15) / 16 * 16;   // two rows per beam + the two selector rows (beamform.cuh)
     q.nks = (row_in + 127) / 128;
+    q.pw = 1;
     q.ntb = (ntime + bfx::BM_MT - 1) / bfx::BM_MT;
     q.nunits = static_cast<long long>(q.ntb) * nchan;
     p->nb2 = q.nb2;
     p->kp = q.nks * ks_bytes;
-    const unsigned stage_bytes = static_cast<unsigned>(ks_bytes / 128) * (bfx::BM_MT * 128u + static_cast<unsigned>(q.nb2) * 128u);
+    unsigned stage_bytes = static_cast<unsigned>(ks_bytes / 128) * (bfx::BM_MT * 128u + static_cast<unsigned>(q.nb2) * 128u);
+    // ci8 spans whose rows are whole multiples of BFX_BM_PW pieces and whose sample count is a multiple of 8 are read through
+    // the 5-d map, BFX_BM_PW pieces per box and K stage -- if at least three such stages fit
+    if (!ci4 && BFX_BM_PW > 1 && row_in % (128 * BFX_BM_PW) == 0 && ntime % 8 == 0 &&
+        3u * BFX_BM_PW * stage_bytes + 1536u + bfx::BM_STG_BYTES <= static_cast<unsigned>(bfx::BM_SMEM_MAX)) {
+        q.pw = BFX_BM_PW;
+        q.nks = row_in / (128 * BFX_BM_PW);
+        stage_bytes *= BFX_BM_PW;
+    }
     // ci4: raw ring of 16 KB tiles beside the operand stages (2 when the stages are at their largest, else 4)
     const unsigned raw_tile = bfx::BM_MT * 128u;
     const unsigned fixed = 1536u + bfx::BM_STG_BYTES;
@@ -207,11 +220,18 @@ int bfBeamformExecute(bfBeamform p, const void* in, void* out, void* stream)
     // span boxes: 128 bytes of a row x 1 channel x 128 samples; rows and samples beyond the span read as zeros
     const bool ci4 = p->dtype == BF_XCORR_CI4;
     CUtensorMap xmap;
-    const cuuint64_t dims[3] = {static_cast<cuuint64_t>(q.row_in), static_cast<cuuint64_t>(p->nchan), static_cast<cuuint64_t>(p->ntime)};
-    const cuuint64_t strides[2] = {static_cast<cuuint64_t>(q.row_in), static_cast<cuuint64_t>(q.row_in) * p->nchan};
+    const cuuint64_t row = static_cast<cuuint64_t>(q.row_in), sample = row * p->nchan;
+    const cuuint64_t dims[3] = {row, static_cast<cuuint64_t>(p->nchan), static_cast<cuuint64_t>(p->ntime)};
+    const cuuint64_t strides[2] = {row, sample};
     const cuuint32_t box[3] = {128u, 1u, static_cast<cuuint32_t>(bfx::BM_MT)};
-    const cuuint32_t estr[3] = {1u, 1u, 1u};
-    const CUresult r = p->encode(&xmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<void*>(in), dims, strides, box, estr,
+    // q.pw > 1: {128 B, sample % 8, row piece, channel, sample / 8}, box {128, 8, pw, 1, BM_MT / 8}
+    const cuuint64_t dims5[5] = {128u, 8u, row / 128u, static_cast<cuuint64_t>(p->nchan), static_cast<cuuint64_t>(p->ntime / 8)};
+    const cuuint64_t strides5[4] = {sample, 128u, row, 8u * sample};
+    const cuuint32_t box5[5] = {128u, 8u, static_cast<cuuint32_t>(q.pw), 1u, static_cast<cuuint32_t>(bfx::BM_MT / 8)};
+    const cuuint32_t estr[5] = {1u, 1u, 1u, 1u, 1u};
+    const CUresult r = q.pw > 1 ? p->encode(&xmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 5, const_cast<void*>(in), dims5, strides5, box5, estr,
+                                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, BFX_BM_PROMO, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE)
+                                : p->encode(&xmap, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<void*>(in), dims, strides, box, estr,
                                  CU_TENSOR_MAP_INTERLEAVE_NONE, ci4 ? CU_TENSOR_MAP_SWIZZLE_NONE : CU_TENSOR_MAP_SWIZZLE_128B,
                                  BFX_BM_PROMO, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) {

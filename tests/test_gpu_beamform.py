@@ -52,7 +52,11 @@ SHAPES = [
     (512, 3, 300, 32),    # station shape: several K stages, ragged tail
     (528, 2, 128, 5),
     (128, 2, 257, 127),   # maximum beam count (2 * 127 + 2 = 256 accumulator columns)
-    (256, 170, 64, 4),    # more units than SMs with a single short sample block
+    (256, 170, 64, 4),    # more units than SMs with a single short sample block (ci8: two-piece span boxes, 5-d map)
+    (512, 3, 296, 32),    # ci8: two-piece span boxes, four K stages, a sample count that is a multiple of 8 but not of 128
+    (256, 6, 1000, 16),   # the same with eight sample blocks
+    (1024, 2, 136, 40),   # wider weight tiles beside the two-piece boxes
+    (384, 4, 264, 9),     # rows of three pieces: no whole number of two-piece boxes, so the 3-d map
 ]
 
 
