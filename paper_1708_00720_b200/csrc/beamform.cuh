@@ -22,7 +22,7 @@
 //
 // Roles (512 threads, one CTA per SM): warp 0 span producer (TMA boxes of 128 span bytes x 128 samples of one channel:
 // ci8 lands 128B-swizzled straight in the operand stage -- two adjacent 128-byte pieces per box through a 5-d view of
-// the span where the shape allows it (rows a multiple of 256 bytes, samples a multiple of 8, three stages fit), which
+// the span where the shape allows it (rows a multiple of 256 bytes, samples a multiple of 8, two stages fit), which
 // the memory system serves much faster when a channel's samples lie pages apart: 76 -> 92 % of the HBM copy peak on
 // BASELINE.json configs[2], 70 -> 102 % on configs[3] (profiles/round2.md) --, ci4 lands raw in a ring), warp 3 weight producer (ci4 only; for
 // ci8 warp 0 loads both), warp 1 MMA issuer, warp 2 TMEM allocator, warps 4..7 epilogue (TMEM -> registers -> shared

@@ -20,6 +20,10 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
 #ifndef BFX_BM_PW
 #define BFX_BM_PW 2
 #endif
+// ... taken when at least this many such stages fit (100 beams on cfg3: two two-piece stages 74 %, five one-piece stages 67 % of the copy peak)
+#ifndef BFX_BM_MINST
+#define BFX_BM_MINST 2u
+#endif
 #ifndef BFX_BM_GROUP_MB
 #define BFX_BM_GROUP_MB 8
 #endif
@@ -127,9 +131,9 @@ int bfBeamformCreate(bfBeamform* plan, int ninputs, int nchan, int ntime, int nb
     p->kp = q.nks * ks_bytes;
     unsigned stage_bytes = static_cast<unsigned>(ks_bytes / 128) * (bfx::BM_MT * 128u + static_cast<unsigned>(q.nb2) * 128u);
     // ci8 spans whose rows are whole multiples of BFX_BM_PW pieces and whose sample count is a multiple of 8 are read through
-    // the 5-d map, BFX_BM_PW pieces per box and K stage -- if at least three such stages fit
+    // the 5-d map, BFX_BM_PW pieces per box and K stage -- if at least BFX_BM_MINST such stages fit
     if (!ci4 && BFX_BM_PW > 1 && row_in % (128 * BFX_BM_PW) == 0 && ntime % 8 == 0 &&
-        3u * BFX_BM_PW * stage_bytes + 1536u + bfx::BM_STG_BYTES <= static_cast<unsigned>(bfx::BM_SMEM_MAX)) {
+        BFX_BM_MINST * BFX_BM_PW * stage_bytes + 1536u + bfx::BM_STG_BYTES <= static_cast<unsigned>(bfx::BM_SMEM_MAX)) {
         q.pw = BFX_BM_PW;
         q.nks = row_in / (128 * BFX_BM_PW);
         stage_bytes *= BFX_BM_PW;

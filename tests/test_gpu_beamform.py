@@ -57,6 +57,7 @@ SHAPES = [
     (256, 6, 1000, 16),   # the same with eight sample blocks
     (1024, 2, 136, 40),   # wider weight tiles beside the two-piece boxes
     (384, 4, 264, 9),     # rows of three pieces: no whole number of two-piece boxes, so the 3-d map
+    (512, 3, 264, 127),   # ci8: the largest weight tiles -- only two two-piece stages fit
 ]
 
 
